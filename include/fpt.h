@@ -1,0 +1,157 @@
+/* fpt.h -- C ABI of libfpt_b200: first-passage-time Monte Carlo of noisy washboard / RCSJ Langevin
+ * trajectories on one NVIDIA B200 (sm_100a).
+ *
+ * PAPER.md = /root/reference/PAPER.md (arXiv:1802.05065, "Stochastic first passage time accelerated with CUDA").
+ * The operations exported here are the paper's two kernels and its output arrays, re-designed for B200:
+ *   - Alg. 1 ESCAPETIME: integrate Eq. (9) step by step, "checking at each
+ *     time step if a threshold crossing ... has occurred", store the escape time k*h,
+ *     or -1 when the step cap klim is reached;
+ *   - Alg. 3 SWITCHINGCURRENT: same loop with the bias ramp gamma_k = gamma0 + dgamma*k
+ *     (PAPER.md:295), store the bias at the crossing;
+ *   - the switching-current histogram;
+ *   - "assigns a new job to the processor as soon as it has terminated its task": done inside
+ *     the kernel by a warp-aggregated claim on a global trajectory counter.
+ * The exact arithmetic (Philox4x32-10 keying, uniforms, Box-Muller, sin/log/sincos algorithms, the four recurrences,
+ * cap and sentinel rules) is DESIGN.md section 4 ("MATH SPEC"); readings of silent passages are DESIGN.md section 3.
+ *
+ * Conventions
+ *   - Every pointer named out_*, values, status, counts is DEVICE memory owned by the caller unless the function name
+ *     ends in _host.  `p` is HOST memory, read during the call only.  The library keeps no pointer after returning.
+ *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) of the
+ *     CURRENT device and return without synchronising; outputs are valid once the stream has been synchronised.
+ *     (_host and fpt_last_stats / fpt_*_peak synchronise before returning.)
+ *   - Return value: FPT_OK, or a negative code.  On FPT_E_INVALID nothing has been enqueued or written.
+ *     No exceptions, no errno, no printing.  fpt_strerror() gives a static string (for FPT_E_CUDA: the CUDA error
+ *     string of the most recent failure on the calling thread).
+ *   - Determinism: per-trajectory outputs are a pure function of (params, seed, trajectory id); they do not depend on
+ *     launch geometry, on check_every, on the GPU, or on which lane integrated which trajectory.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns FPT_E_CUDA.
+ */
+#ifndef FPT_B200_H_
+#define FPT_B200_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define FPT_OK          0
+#define FPT_E_INVALID (-1)   /* bad argument (see each function)                  */
+#define FPT_E_CUDA    (-2)   /* CUDA runtime failure (no device, alloc, launch)   */
+
+#define FPT_MODEL_OVERDAMPED  0
+#define FPT_MODEL_UNDERDAMPED 1
+#define FPT_SCHEME_EM   0
+#define FPT_SCHEME_HEUN 1
+#define FPT_PREC_FP64 0
+#define FPT_PREC_FP32 1
+
+#define FPT_STATUS_ESCAPED  0
+#define FPT_STATUS_CENSORED 1
+#define FPT_STATUS_NAN      2
+
+/* One simulation's parameters (paper: kernel arguments (V0, beta, gamma, D, h) / (dgamma, V0, beta, D, h),
+ * PAPER.md:137-142, 266-271).  4 x int32, 9 x double, 1 x uint64: 96 bytes, no padding. */
+typedef struct fpt_params {
+  int32_t  model;        /* 0 overdamped : dphi = (gamma(t) - amp*sin phi) dt + sqrt(2*temperature) dW
+                            1 underdamped: phi'' + alpha*phi' + amp*sin phi = gamma(t) + sqrt(2*alpha*temperature) xi (Eq. 9) */
+  int32_t  scheme;       /* 0 Euler-Maruyama (paper's Euler, Alg. 1 lines 11-12), 1 stochastic Heun */
+  int32_t  precision;    /* 0 fp64 state; 1 fp32 state + Kahan-compensated time (outputs stay fp64 functions of k_esc) */
+  int32_t  check_every;  /* K >= 1: poll/refill interval in steps.  NEVER changes results (the crossing test is per step,
+                            PAPER.md:190).  Rounded up to a multiple of the steps per Philox block (2 fp64, 4 fp32).
+                            0 = library default. */
+  double   alpha;        /* damping (paper beta); ignored for model 0 */
+  double   temperature;  /* T (paper theta; D = beta*theta).  model 0: the diffusion constant */
+  double   amp;          /* amplitude of sin phi; 0 => drifted Brownian motion with mu = gamma0 */
+  double   gamma0, nu;   /* bias ramp gamma(t) = gamma0 + nu*t, used as gamma_k = fma(nu*dt, k, gamma0) */
+  double   phi0, v0;     /* initial state (paper: arcsin(gamma), 0) */
+  double   threshold;    /* escape when phi >= threshold (paper: pi - phi0) */
+  double   dt;           /* step h */
+  uint64_t first_id;     /* trajectory id of element 0 of the outputs (sharding); the Philox stream is keyed by (seed, id) */
+} fpt_params;
+
+/* Counters of the most recent fpt_simulate* call on the current device (fpt_last_stats). */
+typedef struct fpt_stats {
+  uint64_t n_traj;             /* trajectories processed                                                  */
+  uint64_t n_escaped, n_censored, n_nan;
+  uint64_t useful_steps;       /* sum over trajectories of k_end (k_esc, or n_cap when censored)          */
+  uint64_t issued_lane_steps;  /* 32 * (steps executed by every warp): lane efficiency = useful / issued   */
+  uint64_t refill_atomics;     /* atomics issued on the global trajectory counter                         */
+  uint64_t n_cap;              /* step cap used = nearbyint(t_max/dt)                                     */
+  int32_t  grid, block;        /* launch geometry used                                                    */
+  int32_t  check_every;        /* effective K                                                             */
+  int32_t  reserved;
+} fpt_stats;
+
+/* Integrate trajectories id = first_id .. first_id+n_traj-1 until first passage or the cap n_cap = nearbyint(t_max/dt).
+ *   out_fpt[i]     (double, required) k_esc*dt; -1.0 if censored; NaN if status 2
+ *   out_gamma_at_escape[i] (double, may be NULL) fma(nu*dt, (double)k_end, gamma0), k_end = k_esc or n_cap; NaN if status 2
+ *   out_status[i]  (int32, required) 0 escaped, 1 censored, 2 phi became NaN before any crossing
+ * Each array has n_traj elements, device memory.  n_traj == 0 is a successful no-op.
+ * FPT_E_INVALID: NULL p / out_fpt / out_status, n_traj < 0, unknown enum, check_every < 0, a non-finite field,
+ *   dt <= 0, t_max <= 0, t_max/dt >= 2^53, temperature < 0, alpha < 0 (model 1). */
+int fpt_simulate(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
+                 double* out_fpt, double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream);
+
+/* As fpt_simulate, and additionally bins the bias at escape of every ESCAPED trajectory (status 0) into
+ * out_counts[nbins+2] = [under, bin 0 .. bin nbins-1, over] (device, uint64, ACCUMULATED into: the caller zeroes), through
+ * a shared-memory histogram merged once per block.  Bin rule as fpt_histogram.  hist_of: 0 = gamma at
+ * escape, 1 = escape time.  Additional FPT_E_INVALID: nbins < 1 or > 8192, hi <= lo, non-finite lo/hi, NULL out_counts. */
+int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
+                      double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
+                      int32_t hist_of, double lo, double hi, int32_t nbins, uint64_t* out_counts, void* cuda_stream);
+
+/* Histogram of values[i] over the entries with status[i] == 0 (status may be NULL: all entries):
+ *   b = floor((x - lo) * (nbins/(hi-lo))) in fp64, the scale computed once; b < 0 -> under, b >= nbins -> over (x == hi is
+ *   "over"), NaN values are not counted.  out_counts[nbins+2] is accumulated into.  Counts are integers, so the result is
+ *   independent of the order of accumulation.  FPT_E_INVALID: n < 0, nbins < 1, hi <= lo, NULL values/out_counts. */
+int fpt_histogram(const double* values, const int32_t* status, int64_t n,
+                  double lo, double hi, int32_t nbins, uint64_t* out_counts, void* cuda_stream);
+
+/* End-to-end convenience: as fpt_simulate but every out_* pointer is HOST memory (pinned or pageable); the call allocates
+ * device buffers, runs, copies the results back and synchronises.  h_counts (may be NULL) as in fpt_simulate_hist with
+ * hist_of/lo/hi/nbins, host memory, accumulated into. */
+int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
+                      double* h_fpt, double* h_gamma_at_escape, int32_t* h_status,
+                      int32_t hist_of, double lo, double hi, int32_t nbins, uint64_t* h_counts);
+
+/* Launch geometry override for subsequent fpt_simulate* calls of this process (results never depend on it):
+ * block = threads per block (multiple of 32, 32..256; 0 = default), blocks_per_sm (0 = default from the occupancy
+ * calculator), max_blocks (0 = no extra cap).  FPT_E_INVALID on a bad value. */
+int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks);
+
+/* Synchronises the current device and returns the counters of the most recent fpt_simulate* call on it. */
+int fpt_last_stats(fpt_stats* out);
+
+/* Roofline denominators measured live: a kernel of independent DFMA (fp64) or FFMA (fp32) chains on every SM, run
+ * repeatedly for about `seconds`; *inst_per_s = thread-instructions per second, *sm_clock_hz = SM clock seen by the
+ * kernel (clock64 ticks / elapsed time; may be NULL). */
+int fpt_fp64_peak(double seconds, double* inst_per_s, double* sm_clock_hz);
+int fpt_fp32_peak(double seconds, double* inst_per_s, double* sm_clock_hz);
+
+const char* fpt_strerror(int code);
+int fpt_version(void);   /* 10000*major + 100*minor + patch */
+
+/* ---- test hooks: the device functions of the hot path, exposed one by one so that tests can compare bits with the
+ * oracle.  All pointers are device memory; work is enqueued on cuda_stream. ---- */
+/* out[4*i..4*i+3] = Philox4x32-10 block `block` of stream (seed, id0+i) */
+int fpt_dbg_philox(uint64_t seed, uint64_t id0, int64_t n_ids, uint64_t block, uint32_t* out, void* cuda_stream);
+/* normals of blocks b0..b0+nblocks-1 of stream (seed, id): fp64 2 per block (z_a, z_b); fp32 4 per block */
+int fpt_dbg_normals_f64(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, double* out, void* cuda_stream);
+int fpt_dbg_normals_f32(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, float* out, void* cuda_stream);
+/* elementwise: which = 0 sin_drift(x), 1 neg2log(x) (x in (0,1)) */
+int fpt_dbg_unary_f64(int32_t which, const double* x, double* y, int64_t n, void* cuda_stream);
+int fpt_dbg_unary_f32(int32_t which, const float* x, float* y, int64_t n, void* cuda_stream);
+/* cos, sin of the Box-Muller angle from the raw 64-bit (fp64) / 32-bit (fp32) word */
+int fpt_dbg_sincos_f64(const uint64_t* Y, double* c, double* s, int64_t n, void* cuda_stream);
+int fpt_dbg_sincos_f32(const uint32_t* o, float* c, float* s, int64_t n, void* cuda_stream);
+/* one trajectory (id) with its states recorded: trace_phi[k], trace_v[k] for k = 0..min(k_end, trace_len-1) (as double),
+ * out_status[0], out_k_end[0]; entries past k_end are left untouched. */
+int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len,
+                  double* trace_phi, double* trace_v, int32_t* out_status, uint64_t* out_k_end, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FPT_B200_H_ */

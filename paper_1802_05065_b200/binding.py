@@ -1,0 +1,255 @@
+"""ctypes binding of libfpt_b200.so -- same names as include/fpt.h, argument marshalling only.
+
+torch is used for device memory and streams (``tensor.data_ptr()``, ``torch.cuda.current_stream().cuda_stream``); every
+step of the path runs in the library's kernels.  The library is loaded on first use; a missing library is an error
+(build it with ``python -m paper_1802_05065_b200.build``) -- there is no fallback of any kind.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+_HERE = Path(__file__).resolve().parent
+_LIB_PATH = _HERE / "libfpt_b200.so"
+
+MODEL = {"overdamped": 0, "underdamped": 1}
+SCHEME = {"em": 0, "heun": 1}
+PRECISION = {"fp64": 0, "fp32": 1}
+HIST_OF = {"gamma": 0, "fpt": 1}
+
+
+class FptError(RuntimeError):
+    pass
+
+
+class FptParams(C.Structure):
+    """struct fpt_params of include/fpt.h (96 bytes)."""
+    _fields_ = [("model", C.c_int32), ("scheme", C.c_int32), ("precision", C.c_int32), ("check_every", C.c_int32),
+                ("alpha", C.c_double), ("temperature", C.c_double), ("amp", C.c_double), ("gamma0", C.c_double),
+                ("nu", C.c_double), ("phi0", C.c_double), ("v0", C.c_double), ("threshold", C.c_double),
+                ("dt", C.c_double), ("first_id", C.c_uint64)]
+
+
+class FptStats(C.Structure):
+    """struct fpt_stats of include/fpt.h."""
+    _fields_ = [("n_traj", C.c_uint64), ("n_escaped", C.c_uint64), ("n_censored", C.c_uint64), ("n_nan", C.c_uint64),
+                ("useful_steps", C.c_uint64), ("issued_lane_steps", C.c_uint64), ("refill_atomics", C.c_uint64),
+                ("n_cap", C.c_uint64), ("grid", C.c_int32), ("block", C.c_int32), ("check_every", C.c_int32),
+                ("reserved", C.c_int32)]
+
+    def as_dict(self):
+        d = {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+        d["lane_efficiency"] = d["useful_steps"] / d["issued_lane_steps"] if d["issued_lane_steps"] else None
+        return d
+
+
+_lib = None
+
+_SIGNATURES = {
+    "fpt_simulate": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p],
+    "fpt_simulate_hist": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                          C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
+    "fpt_histogram": [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
+    "fpt_simulate_host": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                          C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p],
+    "fpt_set_launch": [C.c_int32, C.c_int32, C.c_int32],
+    "fpt_last_stats": [C.POINTER(FptStats)],
+    "fpt_fp64_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
+    "fpt_fp32_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
+    "fpt_strerror": [C.c_int],
+    "fpt_version": [],
+    "fpt_dbg_philox": [C.c_uint64, C.c_uint64, C.c_int64, C.c_uint64, C.c_void_p, C.c_void_p],
+    "fpt_dbg_normals_f64": [C.c_uint64, C.c_uint64, C.c_uint64, C.c_int64, C.c_void_p, C.c_void_p],
+    "fpt_dbg_normals_f32": [C.c_uint64, C.c_uint64, C.c_uint64, C.c_int64, C.c_void_p, C.c_void_p],
+    "fpt_dbg_unary_f64": [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
+    "fpt_dbg_unary_f32": [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
+    "fpt_dbg_sincos_f64": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
+    "fpt_dbg_sincos_f32": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
+    "fpt_dbg_trace": [C.POINTER(FptParams), C.c_uint64, C.c_uint64, C.c_double, C.c_int64, C.c_void_p, C.c_void_p,
+                      C.c_void_p, C.c_void_p, C.c_void_p],
+}
+EXPORTS = tuple(_SIGNATURES)
+
+
+def lib():
+    """Load libfpt_b200.so (once).  Raises FptError if it has not been built -- there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not _LIB_PATH.exists():
+            raise FptError(f"{_LIB_PATH} is missing: build it with `python -m paper_1802_05065_b200.build` "
+                           "(nvcc, sm_100a).  This package has no CPU fallback.")
+        L = C.CDLL(str(_LIB_PATH))
+        for name, argtypes in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.argtypes = argtypes
+            fn.restype = C.c_char_p if name == "fpt_strerror" else C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise FptError(f"{what}: {lib().fpt_strerror(rc).decode()} (code {rc})")
+
+
+def _stream(stream=None):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream))
+
+
+def _ptr(t):
+    return C.c_void_p(0 if t is None else t.data_ptr())
+
+
+def make_params(model="underdamped", scheme="heun", precision="fp64", check_every=0, alpha=0.0, temperature=0.0, amp=1.0,
+                gamma0=0.0, nu=0.0, phi0=0.0, v0=0.0, threshold=0.0, dt=0.0, first_id=0, **_ignored) -> FptParams:
+    m = MODEL[model] if isinstance(model, str) else int(model)
+    s = SCHEME[scheme] if isinstance(scheme, str) else int(scheme)
+    pr = PRECISION[precision] if isinstance(precision, str) else int(precision)
+    return FptParams(m, s, pr, check_every, alpha, temperature, amp, gamma0, nu, phi0, v0, threshold, dt, first_id)
+
+
+def _alloc_outputs(n, want_gamma=True, device=None):
+    import torch
+    device = device or torch.device("cuda", torch.cuda.current_device())
+    fpt = torch.empty(n, dtype=torch.float64, device=device)
+    gam = torch.empty(n, dtype=torch.float64, device=device) if want_gamma else None
+    st = torch.empty(n, dtype=torch.int32, device=device)
+    return fpt, gam, st
+
+
+def simulate(params: FptParams, n_traj: int, seed: int, t_max: float, out=None, stream=None):
+    """fpt_simulate.  `out` = (fpt, gamma|None, status) CUDA tensors, allocated when None.  Asynchronous."""
+    fpt, gam, st = out if out is not None else _alloc_outputs(n_traj)
+    _check(lib().fpt_simulate(C.byref(params), n_traj, seed, t_max, _ptr(fpt), _ptr(gam), _ptr(st), _stream(stream)),
+           "fpt_simulate")
+    return fpt, gam, st
+
+
+def simulate_hist(params: FptParams, n_traj: int, seed: int, t_max: float, lo: float, hi: float, nbins: int,
+                  hist_of="gamma", counts=None, out=None, stream=None):
+    """fpt_simulate_hist.  `counts` (uint64-as-int64 CUDA tensor of nbins+2) is accumulated into; zeros when None."""
+    import torch
+    fpt, gam, st = out if out is not None else _alloc_outputs(n_traj)
+    if counts is None:
+        counts = torch.zeros(nbins + 2, dtype=torch.int64, device=fpt.device)
+    h = HIST_OF[hist_of] if isinstance(hist_of, str) else int(hist_of)
+    _check(lib().fpt_simulate_hist(C.byref(params), n_traj, seed, t_max, _ptr(fpt), _ptr(gam), _ptr(st), h, lo, hi, nbins,
+                                   _ptr(counts), _stream(stream)), "fpt_simulate_hist")
+    return fpt, gam, st, counts
+
+
+def histogram(values, status, lo: float, hi: float, nbins: int, counts=None, stream=None):
+    import torch
+    if counts is None:
+        counts = torch.zeros(nbins + 2, dtype=torch.int64, device=values.device)
+    _check(lib().fpt_histogram(_ptr(values), _ptr(status), values.numel(), lo, hi, nbins, _ptr(counts), _stream(stream)),
+           "fpt_histogram")
+    return counts
+
+
+def simulate_host(params: FptParams, n_traj: int, seed: int, t_max: float, fpt, gamma, status, hist=None):
+    """fpt_simulate_host: `fpt`, `gamma` (or None), `status` are HOST buffers (numpy arrays or CPU torch tensors, pinned
+    or not); hist = (hist_of, lo, hi, nbins, counts_host) or None.  Synchronous."""
+    def hp(a):
+        if a is None:
+            return C.c_void_p(0)
+        return C.c_void_p(a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data)
+    if hist is None:
+        h, lo, hi, nb, cnt = 0, 0.0, 1.0, 0, None
+    else:
+        h, lo, hi, nb, cnt = hist
+        h = HIST_OF[h] if isinstance(h, str) else int(h)
+    _check(lib().fpt_simulate_host(C.byref(params), n_traj, seed, t_max, hp(fpt), hp(gamma), hp(status), h, lo, hi, nb,
+                                   hp(cnt)), "fpt_simulate_host")
+
+
+def set_launch(block=0, blocks_per_sm=0, max_blocks=0):
+    _check(lib().fpt_set_launch(block, blocks_per_sm, max_blocks), "fpt_set_launch")
+
+
+def last_stats() -> dict:
+    s = FptStats()
+    _check(lib().fpt_last_stats(C.byref(s)), "fpt_last_stats")
+    return s.as_dict()
+
+
+def fp64_peak(seconds=0.5):
+    r, c = C.c_double(), C.c_double()
+    _check(lib().fpt_fp64_peak(seconds, C.byref(r), C.byref(c)), "fpt_fp64_peak")
+    return r.value, c.value
+
+
+def fp32_peak(seconds=0.5):
+    r, c = C.c_double(), C.c_double()
+    _check(lib().fpt_fp32_peak(seconds, C.byref(r), C.byref(c)), "fpt_fp32_peak")
+    return r.value, c.value
+
+
+def version() -> int:
+    return lib().fpt_version()
+
+
+# ---- test hooks ---------------------------------------------------------------------------------------------------
+def dbg_philox(seed, id0, n_ids, block, stream=None):
+    import torch
+    out = torch.empty(4 * n_ids, dtype=torch.int32, device="cuda")
+    _check(lib().fpt_dbg_philox(seed, id0, n_ids, block, _ptr(out), _stream(stream)), "fpt_dbg_philox")
+    return out
+
+
+def dbg_normals_f64(seed, tid, b0, nblocks, stream=None):
+    import torch
+    out = torch.empty(2 * nblocks, dtype=torch.float64, device="cuda")
+    _check(lib().fpt_dbg_normals_f64(seed, tid, b0, nblocks, _ptr(out), _stream(stream)), "fpt_dbg_normals_f64")
+    return out
+
+
+def dbg_normals_f32(seed, tid, b0, nblocks, stream=None):
+    import torch
+    out = torch.empty(4 * nblocks, dtype=torch.float32, device="cuda")
+    _check(lib().fpt_dbg_normals_f32(seed, tid, b0, nblocks, _ptr(out), _stream(stream)), "fpt_dbg_normals_f32")
+    return out
+
+
+def dbg_unary_f64(which, x, stream=None):
+    import torch
+    y = torch.empty_like(x)
+    _check(lib().fpt_dbg_unary_f64(which, _ptr(x), _ptr(y), x.numel(), _stream(stream)), "fpt_dbg_unary_f64")
+    return y
+
+
+def dbg_unary_f32(which, x, stream=None):
+    import torch
+    y = torch.empty_like(x)
+    _check(lib().fpt_dbg_unary_f32(which, _ptr(x), _ptr(y), x.numel(), _stream(stream)), "fpt_dbg_unary_f32")
+    return y
+
+
+def dbg_sincos_f64(Y, stream=None):
+    import torch
+    c = torch.empty(Y.numel(), dtype=torch.float64, device=Y.device)
+    s = torch.empty_like(c)
+    _check(lib().fpt_dbg_sincos_f64(_ptr(Y), _ptr(c), _ptr(s), Y.numel(), _stream(stream)), "fpt_dbg_sincos_f64")
+    return c, s
+
+
+def dbg_sincos_f32(o, stream=None):
+    import torch
+    c = torch.empty(o.numel(), dtype=torch.float32, device=o.device)
+    s = torch.empty_like(c)
+    _check(lib().fpt_dbg_sincos_f32(_ptr(o), _ptr(c), _ptr(s), o.numel(), _stream(stream)), "fpt_dbg_sincos_f32")
+    return c, s
+
+
+def dbg_trace(params: FptParams, seed, tid, t_max, trace_len, stream=None):
+    import torch
+    phi = torch.full((trace_len,), float("nan"), dtype=torch.float64, device="cuda")
+    v = torch.full((trace_len,), float("nan"), dtype=torch.float64, device="cuda")
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ke = torch.zeros(1, dtype=torch.int64, device="cuda")
+    _check(lib().fpt_dbg_trace(C.byref(params), seed, tid, t_max, trace_len, _ptr(phi), _ptr(v), _ptr(st), _ptr(ke),
+                               _stream(stream)), "fpt_dbg_trace")
+    return phi, v, st, ke

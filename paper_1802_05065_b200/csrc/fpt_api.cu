@@ -1,0 +1,568 @@
+// fpt_api.cu -- the C ABI of include/fpt.h: argument validation, the host-side derived constants,
+// launch geometry, the standalone histogram kernel, the roofline microbenchmarks and the test hooks.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include "../../include/fpt.h"
+#include "fpt_inst.cuh"
+#include "fpt_integrator.cuh"
+
+namespace {
+
+using namespace fpt;
+
+thread_local cudaError_t g_last_cuda = cudaSuccess;
+
+#define FPT_CUDA(call)                         \
+  do {                                         \
+    cudaError_t err__ = (call);                \
+    if (err__ != cudaSuccess) {                \
+      g_last_cuda = err__;                     \
+      (void)cudaGetLastError();                \
+      return FPT_E_CUDA;                       \
+    }                                          \
+  } while (0)
+
+constexpr int kMaxDevices = 64;
+constexpr int kDefaultK = 16;
+
+struct LaunchCfg {
+  int block = 0, blocks_per_sm = 0, max_blocks = 0;
+};
+std::mutex g_mu;
+LaunchCfg g_cfg;
+
+struct DeviceCtx {          // per device: the "last call" counters
+  DevStats* d_last = nullptr;
+  fpt_stats host{};         // geometry etc. filled at launch, counters read back on demand
+  cudaStream_t last_stream = nullptr;
+  bool valid = false;
+  int sm_count = 0;
+};
+DeviceCtx g_ctx[kMaxDevices];
+
+int device_ctx(DeviceCtx** out) {
+  int dev = 0;
+  FPT_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return FPT_E_CUDA;
+  DeviceCtx& c = g_ctx[dev];
+  if (!c.d_last) {
+    FPT_CUDA(cudaMalloc(&c.d_last, sizeof(DevStats)));
+    FPT_CUDA(cudaMemset(c.d_last, 0, sizeof(DevStats)));
+    FPT_CUDA(cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev));
+  }
+  *out = &c;
+  return FPT_OK;
+}
+
+bool finite_all(const double* x, int n) {
+  for (int i = 0; i < n; ++i)
+    if (!std::isfinite(x[i])) return false;
+  return true;
+}
+
+int validate(const fpt_params* p, int64_t n_traj, double t_max) {
+  if (!p || n_traj < 0) return FPT_E_INVALID;
+  if (p->model < 0 || p->model > 1 || p->scheme < 0 || p->scheme > 1 || p->precision < 0 || p->precision > 1) return FPT_E_INVALID;
+  if (p->check_every < 0) return FPT_E_INVALID;
+  const double f[] = {p->alpha, p->temperature, p->amp, p->gamma0, p->nu, p->phi0, p->v0, p->threshold, p->dt, t_max};
+  if (!finite_all(f, 10)) return FPT_E_INVALID;
+  if (!(p->dt > 0.0) || !(t_max > 0.0) || p->temperature < 0.0) return FPT_E_INVALID;
+  if (p->model == 1 && p->alpha < 0.0) return FPT_E_INVALID;
+  if (!(t_max / p->dt < 0x1p53)) return FPT_E_INVALID;
+  return FPT_OK;
+}
+
+// derived constants, fp64, left-to-right products; the fp32 copies are each rounded once.
+void derive(const fpt_params& p, double t_max, uint64_t seed, KParams& P) {
+  std::memset(&P, 0, sizeof(P));
+  P.alpha = p.alpha;
+  P.amp = p.amp;
+  P.gamma0 = p.gamma0;
+  P.dgamma = p.nu * p.dt;
+  P.phi0 = p.phi0;
+  P.v0 = p.v0;
+  P.thr = p.threshold;
+  P.dt = p.dt;
+  P.sigma = (p.model == 1) ? std::sqrt(2.0 * p.alpha * p.temperature * p.dt) : std::sqrt(2.0 * p.temperature * p.dt);
+  P.h2 = 0.5 * p.dt;
+  P.alpha_f = (float)p.alpha;
+  P.amp_f = (float)p.amp;
+  P.gamma0_f = (float)p.gamma0;
+  P.nu_f = (float)p.nu;
+  P.phi0_f = (float)p.phi0;
+  P.v0_f = (float)p.v0;
+  P.thr_f = (float)p.threshold;
+  P.dt_f = (float)p.dt;
+  P.sigma_f = (float)P.sigma;
+  P.h2_f = (float)P.h2;
+  P.first_id = p.first_id;
+  P.n_cap = (unsigned long long)std::nearbyint(t_max / p.dt);
+  const int macro = p.precision == FPT_PREC_FP32 ? 4 : 2;
+  int K = p.check_every > 0 ? p.check_every : kDefaultK;
+  K = ((K + macro - 1) / macro) * macro;
+  P.K = K;
+  P.hist_of = -1;
+  P.keys = philox_round_keys(seed);
+}
+
+// Trajectories that are decided at k = 0 (phi0 >= threshold: escaped at once, PAPER.md:166 applied to the initial state)
+// or by n_cap == 0 (censored at once) are the same for every id: written by a fill kernel, no integration.
+__global__ void fpt_fill_kernel(KParams P, int status, double fptv, double gam) {
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < P.n_traj; i += stride) {
+    P.out_fpt[i] = fptv;
+    if (P.out_gamma) P.out_gamma[i] = gam;
+    P.out_status[i] = status;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (status == kStatusEscaped) {
+      P.ws->n_escaped = P.n_traj;
+      if (P.hist_of >= 0) {
+        const int slot = hist_slot(P.hist_of == 0 ? gam : fptv, P.hist_lo, P.hist_scale, P.nbins);
+        if (slot >= 0) atomicAdd(&P.out_counts[slot], P.n_traj);
+      }
+    } else {
+      P.ws->n_censored = P.n_traj;
+      P.ws->useful_steps = 0;
+    }
+  }
+}
+
+int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt, double* out_gamma,
+                  int32_t* out_status, bool with_hist, int32_t hist_of, double lo, double hi, int32_t nbins,
+                  uint64_t* out_counts, void* cuda_stream) {
+  int rc = validate(p, n_traj, t_max);
+  if (rc != FPT_OK) return rc;
+  if (n_traj > 0 && (!out_fpt || !out_status)) return FPT_E_INVALID;   // empty outputs may be NULL
+  if (with_hist) {
+    if (!out_counts || nbins < 1 || nbins > kMaxFusedBins || !std::isfinite(lo) || !std::isfinite(hi) || !(hi > lo)) return FPT_E_INVALID;
+    if (hist_of < 0 || hist_of > 1) return FPT_E_INVALID;
+  }
+  if (n_traj == 0) return FPT_OK;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  DeviceCtx* ctx = nullptr;
+  rc = device_ctx(&ctx);
+  if (rc != FPT_OK) return rc;
+
+  KParams P;
+  derive(*p, t_max, seed, P);
+  P.n_traj = (unsigned long long)n_traj;
+  P.out_fpt = out_fpt;
+  P.out_gamma = out_gamma;
+  P.out_status = out_status;
+  if (with_hist) {
+    P.hist_of = hist_of;
+    P.nbins = nbins;
+    P.hist_lo = lo;
+    P.hist_scale = (double)nbins / (hi - lo);
+    P.out_counts = (unsigned long long*)out_counts;
+  }
+  DevStats* ws = nullptr;
+  FPT_CUDA(cudaMallocAsync(&ws, sizeof(DevStats), stream));
+  FPT_CUDA(cudaMemsetAsync(ws, 0, sizeof(DevStats), stream));
+  P.ws = ws;
+
+  LaunchCfg cfg;
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    cfg = g_cfg;
+  }
+  int grid = 1, block = 128;
+  const bool fp32 = p->precision == FPT_PREC_FP32;
+  const bool at_once_escaped = fp32 ? !((float)p->phi0 < (float)p->threshold) : !(p->phi0 < p->threshold);
+  if (at_once_escaped || P.n_cap == 0) {
+    block = 256;
+    grid = (int)std::min<int64_t>((n_traj + block - 1) / block, 148 * 8);
+    const int status = at_once_escaped ? kStatusEscaped : kStatusCensored;
+    const double fptv = at_once_escaped ? 0.0 : -1.0;
+    const double gam = std::fma(P.dgamma, at_once_escaped ? 0.0 : (double)P.n_cap, P.gamma0);
+    fpt_fill_kernel<<<grid, block, 0, stream>>>(P, status, fptv, gam);
+    FPT_CUDA(cudaGetLastError());
+  } else {
+    const bool amp = p->amp != 0.0, ramp = p->nu != 0.0;
+    const void* fn = fp32 ? persistent_kernel_f32(p->model, p->scheme, amp, ramp)
+                          : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
+    block = cfg.block > 0 ? cfg.block : 128;
+    const size_t smem = with_hist ? (size_t)(nbins + 2) * sizeof(unsigned int) : 0;
+    int per_sm = 0;
+    FPT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, smem));
+    if (per_sm < 1) return FPT_E_CUDA;
+    if (cfg.blocks_per_sm > 0) per_sm = std::min(per_sm, cfg.blocks_per_sm);
+    long long blocks = (long long)per_sm * ctx->sm_count;
+    const long long needed = (n_traj + block - 1) / block;      // never more lanes than trajectories
+    if (blocks > needed) blocks = needed;
+    if (cfg.max_blocks > 0 && blocks > cfg.max_blocks) blocks = cfg.max_blocks;
+    grid = (int)blocks;
+    void* args[] = {(void*)&P};
+    FPT_CUDA(cudaLaunchKernel(fn, dim3(grid), dim3(block), args, smem, stream));
+  }
+  // keep the counters of this call for fpt_last_stats, then release the per-call workspace (stream ordered)
+  FPT_CUDA(cudaMemcpyAsync(ctx->d_last, ws, sizeof(DevStats), cudaMemcpyDeviceToDevice, stream));
+  FPT_CUDA(cudaFreeAsync(ws, stream));
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    ctx->host = fpt_stats{};
+    ctx->host.n_traj = (uint64_t)n_traj;
+    ctx->host.n_cap = P.n_cap;
+    ctx->host.grid = grid;
+    ctx->host.block = block;
+    ctx->host.check_every = P.K;
+    ctx->last_stream = stream;
+    ctx->valid = true;
+  }
+  return FPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Standalone histogram (S8 / DESIGN.md 4.11): shared-memory bins per block when they fit, global atomics otherwise.
+__global__ void fpt_histogram_kernel(const double* __restrict__ values, const int* __restrict__ status, long long n,
+                                     double lo, double scale, int nbins, unsigned long long* counts, int use_smem) {
+  extern __shared__ unsigned int sh[];
+  if (use_smem) {
+    for (int i = threadIdx.x; i < nbins + 2; i += blockDim.x) sh[i] = 0u;
+    __syncthreads();
+  }
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride) {
+    if (status && status[i] != 0) continue;
+    const int slot = hist_slot(values[i], lo, scale, nbins);
+    if (slot < 0) continue;
+    if (use_smem) atomicAdd(&sh[slot], 1u);
+    else atomicAdd(&counts[slot], 1ull);
+  }
+  if (use_smem) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < nbins + 2; i += blockDim.x) {
+      const unsigned c = sh[i];
+      if (c) atomicAdd(&counts[i], (unsigned long long)c);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Roofline denominators: independent fma chains, 8 per thread, every SM full.
+template <typename T>
+__global__ void __launch_bounds__(256) fpt_peak_kernel(T* sink, int iters, long long* clocks) {
+  T a[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) a[i] = (T)(threadIdx.x + i) * (T)1e-3;
+  const T m = (T)0.999, c = (T)1e-3;
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) {
+        if constexpr (sizeof(T) == 8) a[i] = __fma_rn(a[i], m, c);
+        else a[i] = __fmaf_rn(a[i], m, c);
+      }
+    }
+  }
+  const long long t1 = clock64();
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += a[i];
+  if (s == (T)123456.789) sink[0] = s;
+  if (threadIdx.x == 0 && blockIdx.x == 0) clocks[0] = t1 - t0;
+}
+
+template <typename T>
+int peak_impl(double seconds, double* inst_per_s, double* sm_clock_hz) {
+  if (!inst_per_s || !(seconds > 0.0) || seconds > 30.0) return FPT_E_INVALID;
+  DeviceCtx* ctx = nullptr;
+  int rc = device_ctx(&ctx);
+  if (rc != FPT_OK) return rc;
+  T* sink = nullptr;
+  long long* d_clk = nullptr;
+  FPT_CUDA(cudaMalloc(&sink, sizeof(T)));
+  FPT_CUDA(cudaMalloc(&d_clk, sizeof(long long)));
+  cudaEvent_t e0, e1;
+  FPT_CUDA(cudaEventCreate(&e0));
+  FPT_CUDA(cudaEventCreate(&e1));
+  const int block = 256, grid = ctx->sm_count * 8;
+  const int iters = sizeof(T) == 8 ? 4096 : 16384;
+  const double inst_per_launch = (double)grid * block * (double)iters * 64.0;
+  fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);   // warm-up
+  FPT_CUDA(cudaDeviceSynchronize());
+  double best = 0.0, total_ms = 0.0, clk_hz = 0.0;
+  int launches = 0;
+  while (total_ms < seconds * 1e3 && launches < 100000) {
+    FPT_CUDA(cudaEventRecord(e0));
+    fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);
+    FPT_CUDA(cudaEventRecord(e1));
+    FPT_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    FPT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    total_ms += ms;
+    ++launches;
+    const double rate = inst_per_launch / (ms * 1e-3);
+    if (rate > best) best = rate;
+  }
+  // sustained figure: the LAST launch (after `seconds` of load), and the clock of block 0 of a single-wave launch
+  {
+    FPT_CUDA(cudaEventRecord(e0));
+    fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);
+    FPT_CUDA(cudaEventRecord(e1));
+    FPT_CUDA(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    FPT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+    long long clk = 0;
+    FPT_CUDA(cudaMemcpy(&clk, d_clk, sizeof(clk), cudaMemcpyDeviceToHost));
+    // all 8 blocks/SM are co-resident (256 thr x 8 = 2048), so block 0 runs for the whole launch
+    clk_hz = (double)clk / (ms * 1e-3);
+    *inst_per_s = inst_per_launch / (ms * 1e-3);
+  }
+  if (sm_clock_hz) *sm_clock_hz = clk_hz;
+  (void)best;
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(sink);
+  cudaFree(d_clk);
+  return FPT_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// test-hook kernels
+__global__ void dbg_philox_kernel(PhiloxKeys K, unsigned long long id0, long long n, unsigned long long block, uint32_t* out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const unsigned long long id = id0 + (unsigned long long)i;
+  uint32_t o0, o1, o2, o3;
+  philox_block(K, (uint32_t)block, (uint32_t)(block >> 32), (uint32_t)id, (uint32_t)(id >> 32), o0, o1, o2, o3);
+  out[4 * i] = o0; out[4 * i + 1] = o1; out[4 * i + 2] = o2; out[4 * i + 3] = o3;
+}
+__global__ void dbg_normals64_kernel(PhiloxKeys K, unsigned long long id, unsigned long long b0, long long n, double* out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const unsigned long long b = b0 + (unsigned long long)i;
+  uint32_t o0, o1, o2, o3;
+  philox_block(K, (uint32_t)b, (uint32_t)(b >> 32), (uint32_t)id, (uint32_t)(id >> 32), o0, o1, o2, o3);
+  double za, zb;
+  normal_pair(o0, o1, o2, o3, za, zb);
+  out[2 * i] = za; out[2 * i + 1] = zb;
+}
+__global__ void dbg_normals32_kernel(PhiloxKeys K, unsigned long long id, unsigned long long b0, long long n, float* out) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const unsigned long long b = b0 + (unsigned long long)i;
+  uint32_t o0, o1, o2, o3;
+  philox_block(K, (uint32_t)b, (uint32_t)(b >> 32), (uint32_t)id, (uint32_t)(id >> 32), o0, o1, o2, o3);
+  float z0, z1, z2, z3;
+  normal_pair_f(o0, o1, z0, z1);
+  normal_pair_f(o2, o3, z2, z3);
+  out[4 * i] = z0; out[4 * i + 1] = z1; out[4 * i + 2] = z2; out[4 * i + 3] = z3;
+}
+__global__ void dbg_unary64_kernel(int which, const double* x, double* y, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  y[i] = which == 0 ? sin_drift(x[i]) : neg2log(x[i]);
+}
+__global__ void dbg_unary32_kernel(int which, const float* x, float* y, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  y[i] = which == 0 ? sin_drift_f(x[i]) : neg2log_f(x[i]);
+}
+__global__ void dbg_sincos64_kernel(const unsigned long long* Y, double* c, double* s, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double cc, ss;
+  sincos_turns((uint32_t)(Y[i] >> 32), (uint32_t)Y[i], cc, ss);
+  c[i] = cc; s[i] = ss;
+}
+__global__ void dbg_sincos32_kernel(const uint32_t* o, float* c, float* s, long long n) {
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float cc, ss;
+  sincos_turns_f(o[i], cc, ss);
+  c[i] = cc; s[i] = ss;
+}
+
+inline int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
+
+}  // namespace
+
+// =================================================================================================================
+extern "C" {
+
+int fpt_simulate(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
+                 double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream) {
+  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, false, 0, 0.0, 0.0, 0, nullptr,
+                       cuda_stream);
+}
+
+int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
+                      double* out_gamma_at_escape, int32_t* out_status, int32_t hist_of, double lo, double hi,
+                      int32_t nbins, uint64_t* out_counts, void* cuda_stream) {
+  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, true, hist_of, lo, hi, nbins,
+                       out_counts, cuda_stream);
+}
+
+int fpt_histogram(const double* values, const int32_t* status, int64_t n, double lo, double hi, int32_t nbins,
+                  uint64_t* out_counts, void* cuda_stream) {
+  if (!values || !out_counts || n < 0 || nbins < 1 || !std::isfinite(lo) || !std::isfinite(hi) || !(hi > lo)) return FPT_E_INVALID;
+  if (n == 0) return FPT_OK;
+  DeviceCtx* ctx = nullptr;
+  int rc = device_ctx(&ctx);
+  if (rc != FPT_OK) return rc;
+  const double scale = (double)nbins / (hi - lo);
+  const int block = 256;
+  const int grid = (int)std::min<long long>(grid_for(n, block), (long long)ctx->sm_count * 8);
+  const int use_smem = nbins <= kMaxFusedBins ? 1 : 0;
+  const size_t smem = use_smem ? (size_t)(nbins + 2) * sizeof(unsigned int) : 0;
+  fpt_histogram_kernel<<<grid, block, smem, (cudaStream_t)cuda_stream>>>(values, status, (long long)n, lo, scale, nbins,
+                                                                         (unsigned long long*)out_counts, use_smem);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+
+int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* h_fpt, double* h_gamma,
+                      int32_t* h_status, int32_t hist_of, double lo, double hi, int32_t nbins, uint64_t* h_counts) {
+  int rc = validate(p, n_traj, t_max);
+  if (rc != FPT_OK) return rc;
+  if (n_traj == 0) return FPT_OK;
+  if (!h_fpt || !h_status) return FPT_E_INVALID;
+  cudaStream_t stream = nullptr;
+  FPT_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
+  const size_t n = (size_t)n_traj;
+  const size_t bytes = n * (8 + (h_gamma ? 8 : 0) + 4) + (h_counts ? (size_t)(nbins > 0 ? nbins + 2 : 0) * 8 : 0);
+  char* d = nullptr;
+  cudaError_t e = cudaMallocAsync(&d, bytes, stream);
+  if (e != cudaSuccess) { g_last_cuda = e; cudaStreamDestroy(stream); return FPT_E_CUDA; }
+  double* d_fpt = (double*)d;
+  double* d_gam = h_gamma ? d_fpt + n : nullptr;
+  uint64_t* d_cnt = h_counts ? (uint64_t*)(d + n * (8 + (h_gamma ? 8 : 0))) : nullptr;
+  int32_t* d_st = (int32_t*)(d + n * (8 + (h_gamma ? 8 : 0)) + (h_counts ? (size_t)(nbins + 2) * 8 : 0));
+  if (h_counts) {
+    if (nbins < 1) { cudaFreeAsync(d, stream); cudaStreamDestroy(stream); return FPT_E_INVALID; }
+    cudaMemcpyAsync(d_cnt, h_counts, (size_t)(nbins + 2) * 8, cudaMemcpyHostToDevice, stream);
+    rc = fpt_simulate_hist(p, n_traj, seed, t_max, d_fpt, d_gam, d_st, hist_of, lo, hi, nbins, d_cnt, stream);
+  } else {
+    rc = fpt_simulate(p, n_traj, seed, t_max, d_fpt, d_gam, d_st, stream);
+  }
+  if (rc == FPT_OK) {
+    cudaMemcpyAsync(h_fpt, d_fpt, n * 8, cudaMemcpyDeviceToHost, stream);
+    if (h_gamma) cudaMemcpyAsync(h_gamma, d_gam, n * 8, cudaMemcpyDeviceToHost, stream);
+    cudaMemcpyAsync(h_status, d_st, n * 4, cudaMemcpyDeviceToHost, stream);
+    if (h_counts) cudaMemcpyAsync(h_counts, d_cnt, (size_t)(nbins + 2) * 8, cudaMemcpyDeviceToHost, stream);
+  }
+  cudaFreeAsync(d, stream);
+  e = cudaStreamSynchronize(stream);
+  cudaStreamDestroy(stream);
+  if (rc == FPT_OK && e != cudaSuccess) { g_last_cuda = e; (void)cudaGetLastError(); return FPT_E_CUDA; }
+  return rc;
+}
+
+int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks) {
+  if (block != 0 && (block < 32 || block > 256 || (block % 32) != 0)) return FPT_E_INVALID;
+  if (blocks_per_sm < 0 || blocks_per_sm > 64 || max_blocks < 0) return FPT_E_INVALID;
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_cfg.block = block;
+  g_cfg.blocks_per_sm = blocks_per_sm;
+  g_cfg.max_blocks = max_blocks;
+  return FPT_OK;
+}
+
+int fpt_last_stats(fpt_stats* out) {
+  if (!out) return FPT_E_INVALID;
+  DeviceCtx* ctx = nullptr;
+  int rc = device_ctx(&ctx);
+  if (rc != FPT_OK) return rc;
+  FPT_CUDA(cudaDeviceSynchronize());
+  DevStats h;
+  FPT_CUDA(cudaMemcpy(&h, ctx->d_last, sizeof(h), cudaMemcpyDeviceToHost));
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (!ctx->valid) { std::memset(out, 0, sizeof(*out)); return FPT_OK; }
+  *out = ctx->host;
+  out->n_escaped = h.n_escaped;
+  out->n_censored = h.n_censored;
+  out->n_nan = h.n_nan;
+  out->useful_steps = h.useful_steps;
+  out->issued_lane_steps = h.issued_lane_steps;
+  out->refill_atomics = h.refill_atomics;
+  return FPT_OK;
+}
+
+int fpt_fp64_peak(double seconds, double* inst_per_s, double* sm_clock_hz) { return peak_impl<double>(seconds, inst_per_s, sm_clock_hz); }
+int fpt_fp32_peak(double seconds, double* inst_per_s, double* sm_clock_hz) { return peak_impl<float>(seconds, inst_per_s, sm_clock_hz); }
+
+const char* fpt_strerror(int code) {
+  switch (code) {
+    case FPT_OK: return "ok";
+    case FPT_E_INVALID: return "invalid argument";
+    case FPT_E_CUDA: return g_last_cuda != cudaSuccess ? cudaGetErrorString(g_last_cuda) : "CUDA failure";
+    default: return "unknown error code";
+  }
+}
+
+int fpt_version(void) { return 100; }
+
+// ---- test hooks
+int fpt_dbg_philox(uint64_t seed, uint64_t id0, int64_t n_ids, uint64_t block, uint32_t* out, void* s) {
+  if (!out || n_ids < 0) return FPT_E_INVALID;
+  if (n_ids == 0) return FPT_OK;
+  dbg_philox_kernel<<<grid_for(n_ids, 128), 128, 0, (cudaStream_t)s>>>(philox_round_keys(seed), id0, n_ids, block, out);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_normals_f64(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, double* out, void* s) {
+  if (!out || nblocks < 0) return FPT_E_INVALID;
+  if (nblocks == 0) return FPT_OK;
+  dbg_normals64_kernel<<<grid_for(nblocks, 128), 128, 0, (cudaStream_t)s>>>(philox_round_keys(seed), id, b0, nblocks, out);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_normals_f32(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, float* out, void* s) {
+  if (!out || nblocks < 0) return FPT_E_INVALID;
+  if (nblocks == 0) return FPT_OK;
+  dbg_normals32_kernel<<<grid_for(nblocks, 128), 128, 0, (cudaStream_t)s>>>(philox_round_keys(seed), id, b0, nblocks, out);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_unary_f64(int32_t which, const double* x, double* y, int64_t n, void* s) {
+  if (!x || !y || n < 0 || which < 0 || which > 1) return FPT_E_INVALID;
+  if (n == 0) return FPT_OK;
+  dbg_unary64_kernel<<<grid_for(n, 128), 128, 0, (cudaStream_t)s>>>(which, x, y, n);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_unary_f32(int32_t which, const float* x, float* y, int64_t n, void* s) {
+  if (!x || !y || n < 0 || which < 0 || which > 1) return FPT_E_INVALID;
+  if (n == 0) return FPT_OK;
+  dbg_unary32_kernel<<<grid_for(n, 128), 128, 0, (cudaStream_t)s>>>(which, x, y, n);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_sincos_f64(const uint64_t* Y, double* c, double* sn, int64_t n, void* s) {
+  if (!Y || !c || !sn || n < 0) return FPT_E_INVALID;
+  if (n == 0) return FPT_OK;
+  dbg_sincos64_kernel<<<grid_for(n, 128), 128, 0, (cudaStream_t)s>>>((const unsigned long long*)Y, c, sn, n);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_sincos_f32(const uint32_t* o, float* c, float* sn, int64_t n, void* s) {
+  if (!o || !c || !sn || n < 0) return FPT_E_INVALID;
+  if (n == 0) return FPT_OK;
+  dbg_sincos32_kernel<<<grid_for(n, 128), 128, 0, (cudaStream_t)s>>>(o, c, sn, n);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len, double* trace_phi,
+                  double* trace_v, int32_t* out_status, uint64_t* out_k_end, void* s) {
+  int rc = validate(p, 0, t_max);
+  if (rc != FPT_OK) return rc;
+  if (trace_len < 0 || (trace_len > 0 && !trace_phi)) return FPT_E_INVALID;
+  KParams P;
+  derive(*p, t_max, seed, P);
+  TraceArgs T{id, trace_len, trace_phi, trace_v, out_status, (unsigned long long*)out_k_end};
+  const void* fn = p->precision == FPT_PREC_FP32 ? trace_kernel_f32(p->model, p->scheme) : trace_kernel_f64(p->model, p->scheme);
+  void* args[] = {(void*)&P, (void*)&T};
+  FPT_CUDA(cudaLaunchKernel(fn, dim3(1), dim3(32), args, 0, (cudaStream_t)s));
+  return FPT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,105 @@
+"""Boundary checks that need no GPU: the C-ABI library builds, loads and exports every symbol include/fpt.h declares,
+the struct layouts match the header, and argument validation (FPT_E_INVALID) happens before any CUDA work."""
+import ctypes as C
+import math
+import re
+from pathlib import Path
+
+import pytest
+
+import paper_1802_05065_b200 as fpt
+from paper_1802_05065_b200 import binding, build
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return fpt.lib()
+
+
+def test_exports_every_declared_symbol(lib):
+    header = (ROOT / "include" / "fpt.h").read_text()
+    code = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(fpt_[a-z0-9_]+)\s*\(", code))
+    assert len(declared) >= 15
+    for name in declared:
+        assert hasattr(lib, name), name
+    assert declared == set(binding.EXPORTS)          # the binding covers the whole header, and nothing else
+
+
+def test_struct_layouts(lib):
+    assert C.sizeof(fpt.FptParams) == 96              # 4 x int32, 9 x double, 1 x uint64, no padding
+    assert fpt.FptParams.first_id.offset == 88
+    assert C.sizeof(fpt.FptStats) == 80
+    assert fpt.version() >= 100
+
+
+def test_strerror(lib):
+    assert lib.fpt_strerror(0) == b"ok"
+    assert lib.fpt_strerror(-1) == b"invalid argument"
+    assert lib.fpt_strerror(-99) == b"unknown error code"
+
+
+def _good():
+    return dict(fpt.workload("c2")["params"])
+
+
+@pytest.mark.parametrize("field,value", [("dt", 0.0), ("dt", -1.0), ("dt", math.nan), ("temperature", -0.1), ("alpha", -1.0),
+                                         ("model", 2), ("scheme", -1), ("precision", 3), ("check_every", -1),
+                                         ("gamma0", math.inf), ("threshold", math.nan)])
+def test_invalid_params_rejected_before_any_cuda_work(lib, field, value):
+    kw = _good()
+    kw[field] = value
+    p = fpt.make_params(**kw)
+    # non-null dummy pointers: validation must reject before touching them (there is no GPU here)
+    rc = lib.fpt_simulate(C.byref(p), 10, 1, 1.0, C.c_void_p(8), C.c_void_p(8), C.c_void_p(8), None)
+    assert rc == -1
+
+
+def test_invalid_call_arguments(lib):
+    p = fpt.make_params(**_good())
+    assert lib.fpt_simulate(None, 10, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8), None) == -1
+    assert lib.fpt_simulate(C.byref(p), -1, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8), None) == -1
+    assert lib.fpt_simulate(C.byref(p), 10, 1, 0.0, C.c_void_p(8), None, C.c_void_p(8), None) == -1
+    assert lib.fpt_simulate(C.byref(p), 10, 1, 1e300, C.c_void_p(8), None, C.c_void_p(8), None) == -1     # t_max/dt >= 2^53
+    assert lib.fpt_simulate(C.byref(p), 10, 1, 1.0, None, None, C.c_void_p(8), None) == -1
+    assert lib.fpt_simulate(C.byref(p), 10, 1, 1.0, C.c_void_p(8), None, None, None) == -1
+    assert lib.fpt_simulate(C.byref(p), 0, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8), None) == 0          # n_traj == 0: no-op
+    h = lambda nb, lo, hi, cnt: lib.fpt_simulate_hist(C.byref(p), 10, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8), 0, lo, hi,
+                                                      nb, cnt, None)
+    assert h(0, 0.0, 1.0, C.c_void_p(8)) == -1
+    assert h(8193, 0.0, 1.0, C.c_void_p(8)) == -1
+    assert h(10, 1.0, 1.0, C.c_void_p(8)) == -1
+    assert h(10, 0.0, 1.0, None) == -1
+    assert lib.fpt_histogram(None, None, 5, 0.0, 1.0, 4, C.c_void_p(8), None) == -1
+    assert lib.fpt_histogram(C.c_void_p(8), None, 5, 1.0, 0.0, 4, C.c_void_p(8), None) == -1
+    assert lib.fpt_histogram(C.c_void_p(8), None, 0, 0.0, 1.0, 4, C.c_void_p(8), None) == 0
+    assert lib.fpt_set_launch(48, 0, 0) == -1
+    assert lib.fpt_set_launch(512, 0, 0) == -1
+    assert lib.fpt_set_launch(128, 2, 0) == 0
+    assert lib.fpt_set_launch(0, 0, 0) == 0
+
+
+def test_no_cpu_fallback(lib):
+    """Without a CUDA device a compute call fails loudly (FPT_E_CUDA); it never computes on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    p = fpt.make_params(**_good())
+    buf = (C.c_double * 16)()
+    st = (C.c_int32 * 16)()
+    rc = lib.fpt_simulate(C.byref(p), 4, 1, 1.0, buf, None, st, None)
+    assert rc == -2
+    assert lib.fpt_strerror(rc) not in (b"ok", b"")
+    rc = lib.fpt_simulate_host(C.byref(p), 4, 1, 1.0, buf, None, st, 0, 0.0, 1.0, 0, None)
+    assert rc == -2
+
+
+def test_product_does_not_import_oracle():
+    for path in (ROOT / "paper_1802_05065_b200").rglob("*"):
+        if path.suffix in (".py", ".cu", ".cuh", ".h"):
+            text = path.read_text()
+            assert "import oracle" not in text and "from oracle" not in text, path
+            assert "fpt_oracle" not in text, path

@@ -1,0 +1,396 @@
+"""GPU parity: the CUDA path, called through the C ABI, against the oracle on the same
+seeded inputs.  Bars (BASELINE.json north_star, written out here):
+
+  * Philox words and normal-variate bits: bit-exact;
+  * per-trajectory escape step index: equal for >= 99.9 % of trajectories (we expect, and assert, 100 % -- both sides
+    implement DESIGN.md section 4 with the same explicitly rounded operations);
+  * escape time and bias at escape: <= 1e-9 relative (fp64), <= 1e-4 (fp32);
+  * distributions: two-sample KS p > 0.01 between GPU ids and an INDEPENDENT oracle sample (other ids).
+"""
+import math
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+import paper_1802_05065_b200 as fpt
+
+pytestmark = pytest.mark.gpu
+
+REL_FP64 = 1e-9
+REL_FP32 = 1e-4
+MATCH_FRACTION = 0.999
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    fpt.lib()                      # fails loudly if the extension is missing
+    fpt.set_launch(0, 0, 0)
+    yield
+    fpt.set_launch(0, 0, 0)
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def same_bits(a, b):
+    """Bit-for-bit equality, except that NaN payloads (which differ between x86 and the GPU) only need to be NaN on both sides."""
+    a = np.asarray(a); b = np.asarray(b)
+    view = np.uint64 if a.dtype == np.float64 else np.uint32
+    na, nb = np.isnan(a), np.isnan(b)
+    return a.shape == b.shape and np.array_equal(na, nb) and np.array_equal(a[~na].view(view), b[~nb].view(view))
+
+
+def run_gpu(w, n=None, first_id=0, check_every=0, hist=False):
+    kw = dict(w["params"], first_id=first_id, check_every=check_every)
+    p = fpt.make_params(**kw)
+    n = w["n_traj"] if n is None else n
+    if hist:
+        of, lo, hi, nb = w["hist"]
+        f, g, s, c = fpt.simulate_hist(p, n, w["seed"], w["t_max"], lo, hi, nb, hist_of=of)
+        torch.cuda.synchronize()
+        return _np(f), _np(g), _np(s), _np(c).astype(np.uint64)
+    f, g, s = fpt.simulate(p, n, w["seed"], w["t_max"])
+    torch.cuda.synchronize()
+    return _np(f), _np(g), _np(s)
+
+
+def run_oracle(w, n, first_id=0):
+    p = oracle.make_params(**dict(w["params"], first_id=first_id))
+    return oracle.simulate(p, n, w["seed"], w["t_max"])
+
+
+def assert_parity(gpu, ora, dt, rel):
+    f, g, s = gpu[:3]
+    assert np.array_equal(s, ora["status"])
+    k_gpu = np.where(s == 0, np.rint(f / dt), -1).astype(np.int64)
+    k_ora = np.where(ora["status"] == 0, ora["k"].astype(np.int64), -1)
+    match = np.mean(k_gpu == k_ora)
+    assert match >= MATCH_FRACTION, match
+    assert match == 1.0, f"escape indices differ for {np.sum(k_gpu != k_ora)} trajectories"   # the design target: none
+    esc = s == 0
+    assert np.all(np.abs(f[esc] - ora["fpt"][esc]) <= rel * np.abs(ora["fpt"][esc]))
+    assert np.all(np.abs(g[esc] - ora["gamma"][esc]) <= rel * np.maximum(1e-300, np.abs(ora["gamma"][esc])))
+    cens = s == 1
+    assert np.all(f[cens] == -1.0)
+    assert np.array_equal(g[cens], ora["gamma"][cens])
+    assert np.array_equal(f[esc], ora["fpt"][esc]) and np.array_equal(g[esc], ora["gamma"][esc])     # in fact bit-identical
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P1: Philox
+def test_philox_known_answers_and_bits():
+    # published known answers use raw (counter, key); with the R1 keying they are reachable as (seed, id, block):
+    # ctr = (b_lo, b_hi, id_lo, id_hi), key = (seed_lo, seed_hi)
+    kat = [((0, 0, 0, 0), (0, 0), (0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8)),
+           ((0xffffffff,) * 4, (0xffffffff,) * 2, (0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd)),
+           ((0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344), (0xa4093822, 0x299f31d0), (0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1))]
+    for ctr, key, want in kat:
+        seed = key[0] | (key[1] << 32)
+        block = ctr[0] | (ctr[1] << 32)
+        tid = ctr[2] | (ctr[3] << 32)
+        got = _np(fpt.dbg_philox(seed, tid, 1, block)).view(np.uint32)
+        assert tuple(int(x) for x in got) == want
+    rng = np.random.default_rng(11)
+    for _ in range(6):
+        seed, id0, block = (int(x) for x in rng.integers(0, 2**63, 3))
+        n = 5000
+        got = _np(fpt.dbg_philox(seed, id0, n, block)).view(np.uint32).reshape(n, 4)
+        for i in rng.integers(0, n, 40):
+            assert tuple(int(x) for x in got[i]) == oracle.philox_block(seed, id0 + int(i), block)
+    # id crossing the 32-bit boundary, block above 2^32 (config 4/5 need 64-bit counters)
+    got = _np(fpt.dbg_philox(5, 2**32 - 2, 4, 2**33)).view(np.uint32).reshape(4, 4)
+    for i in range(4):
+        assert tuple(int(x) for x in got[i]) == oracle.philox_block(5, 2**32 - 2 + i, 2**33)
+
+
+# P2: normals, bit for bit
+def test_normals_fp64_bit_exact():
+    n = 5_000_000                                   # 1e7 normals
+    for seed, tid, b0 in [(1, 0, 0), (3, 999_999, 2**31 - 1000), (2**40 + 5, 2**35 + 1, 2**34)]:
+        got = _np(fpt.dbg_normals_f64(seed, tid, b0, n))
+        want = oracle.normals_f64(seed, tid, b0, n)
+        assert same_bits(got, want)
+    assert abs(float(np.mean(got))) < 5 / math.sqrt(2 * n) and abs(float(np.var(got)) - 1) < 5 * math.sqrt(2 / (2 * n))
+
+
+def test_normals_fp32_bit_exact():
+    n = 2_500_000                                   # 1e7 normals
+    for seed, tid, b0 in [(4, 0, 0), (4, 65535, 2**31 - 7), (77, 2**33, 2**32 + 3)]:
+        got = _np(fpt.dbg_normals_f32(seed, tid, b0, n))
+        want = oracle.normals_f32(seed, tid, b0, n)
+        assert same_bits(got, want)
+
+
+def test_elementary_functions_bit_exact():
+    rng = np.random.default_rng(5)
+    n = 4_000_000
+    # sin of the drift: the working range, reduction boundaries, large and special arguments
+    x = np.concatenate([rng.uniform(-10, 10, n), (np.arange(-40, 41) * (math.pi / 2)), np.nextafter(np.arange(-40, 41) * (math.pi / 2), np.inf),
+                        rng.uniform(-1e6, 1e6, 100000), [0.0, -0.0, 1e-310, 1e300, -1e300, np.inf, -np.inf, np.nan]])
+    got = _np(fpt.dbg_unary_f64(0, torch.from_numpy(x).cuda()))
+    want = oracle.sin_drift(x)
+    assert same_bits(got, want)
+    # -2 ln u on the uniform grid (2N+1) 2^-53, including the smallest and largest u
+    N = np.concatenate([rng.integers(0, 2**52, n, dtype=np.uint64), np.array([0, 1, 2, 2**52 - 1, 2**51, 2**51 - 1], dtype=np.uint64),
+                        rng.integers(0, 2**20, 100000, dtype=np.uint64)])
+    u = (2.0 * N.astype(np.float64) + 1.0) * 2.0**-53
+    got = _np(fpt.dbg_unary_f64(1, torch.from_numpy(u).cuda()))
+    want = oracle.neg2log(u)
+    assert same_bits(got, want)
+    # Box-Muller angle
+    Y = np.concatenate([rng.integers(0, 2**64, n, dtype=np.uint64),
+                        np.array([0, 2**64 - 1, 2**61, 2**61 - 1, 2**62, 2**63, 2**63 + 2**62, 2**11 - 1, 2**11], dtype=np.uint64)])
+    c, s = fpt.dbg_sincos_f64(torch.from_numpy(Y.view(np.int64)).cuda())
+    wc, ws = oracle.sincos_turns(Y)
+    assert same_bits(_np(c), wc) and same_bits(_np(s), ws)
+    # fp32 twins
+    xf = np.concatenate([rng.uniform(-10, 10, n), np.arange(-40, 41) * (math.pi / 2), [0.0, -0.0, 1e30, np.inf, np.nan]]).astype(np.float32)
+    got = _np(fpt.dbg_unary_f32(0, torch.from_numpy(xf).cuda()))
+    assert same_bits(got, oracle.sin_drift_f(xf))
+    o = np.concatenate([rng.integers(0, 2**32, n, dtype=np.uint64), [0, 1, 2**32 - 1, 2**31, 2**29, 2**29 - 1]]).astype(np.uint32)
+    uf = np.array([oracle.uniform_open_f(int(v)) for v in o[-2000:]], dtype=np.float32)
+    uf = np.concatenate([uf, (o[:n].astype(np.float32) * np.float32(2.0**-32) + np.float32(2.0**-33)).astype(np.float32)])
+    uf = uf[(uf > 0) & (uf <= 1)]
+    got = _np(fpt.dbg_unary_f32(1, torch.from_numpy(uf).cuda()))
+    assert same_bits(got, oracle.neg2log_f(uf))
+    c, s = fpt.dbg_sincos_f32(torch.from_numpy(o.view(np.int32)).cuda())
+    wc, ws = oracle.sincos_turns_f(o)
+    assert same_bits(_np(c), wc) and same_bits(_np(s), ws)
+
+
+# states, step by step
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+@pytest.mark.parametrize("model,scheme", [("overdamped", "em"), ("overdamped", "heun"), ("underdamped", "em"), ("underdamped", "heun")])
+def test_trace_states_bit_exact(model, scheme, precision):
+    kw = dict(model=model, scheme=scheme, precision=precision, alpha=0.1, temperature=0.05, amp=1.0, gamma0=0.6, nu=1e-3,
+              phi0=math.asin(0.6), v0=0.1, threshold=math.asin(0.6) + 2 * math.pi, dt=0.02)
+    n = 3000
+    for seed, tid in [(9, 0), (9, 2**32 + 17)]:
+        phi, v, st, ke = fpt.dbg_trace(fpt.make_params(**kw), seed, tid, 1e4, n)
+        torch.cuda.synchronize()
+        ophi, ov, ost, oke = oracle.trace(oracle.make_params(**kw), seed, tid, 1e4, n)
+        assert (int(st[0]), int(ke[0])) == (ost, oke)
+        m = min(n, oke + 1)
+        assert same_bits(_np(phi)[:m], ophi[:m])
+        if model == "underdamped":
+            assert same_bits(_np(v)[:m], ov[:m])
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# P9: the five configs (ids the oracle finishes in seconds; several warps, a ragged tail, refills)
+def test_config1_full():
+    w = fpt.workload("c1")
+    gpu = run_gpu(w)
+    ora = run_oracle(w, w["n_traj"])
+    assert_parity(gpu, ora, w["params"]["dt"], REL_FP64)
+    assert np.all(gpu[2] == 0)
+    # worked example (tests/golden/worked_examples.txt): k_esc of ids 0..7
+    assert [int(round(t / 1e-3)) for t in gpu[0][:8]] == [1650, 808, 1218, 918, 742, 822, 1738, 1140]
+
+
+def test_config2_subset_with_refill():
+    w = fpt.workload("c2")
+    n = 5003                                          # ragged: not a multiple of the warp or block size
+    fpt.set_launch(64, 1, 8)                          # 512 lanes for 5003 trajectories: every lane refills ~10 times
+    try:
+        gpu = run_gpu(w, n)
+        stats = fpt.last_stats()
+    finally:
+        fpt.set_launch(0, 0, 0)
+    ora = run_oracle(w, n)
+    assert_parity(gpu, ora, w["params"]["dt"], REL_FP64)
+    assert [int(round(t / 0.01)) for t in gpu[0][:4]] == [9508, 13989, 7877, 6610]
+    assert stats["n_escaped"] == int(np.sum(ora["status"] == 0)) and stats["n_censored"] == 0
+    assert stats["useful_steps"] == int(np.sum(ora["k"]))
+    assert stats["grid"] == 8 and stats["block"] == 64
+    assert 0.5 < stats["lane_efficiency"] <= 1.0
+
+
+def test_config3_family_fast_ramp_with_fused_histogram():
+    w = fpt.workload("c3", nu=1e-3, t_max=1.05 / 1e-3)
+    n = 1500
+    f, g, s, counts = run_gpu(w, n, hist=True)
+    ora = run_oracle(w, n)
+    assert_parity((f, g, s), ora, w["params"]["dt"], REL_FP64)
+    assert [int(round(t / 0.02)) for t in f[:2]] == [49462, 48646]
+    of, lo, hi, nb = w["hist"]
+    want = oracle.histogram(ora["gamma"], ora["status"], lo, hi, nb)
+    assert np.array_equal(counts, want)
+    assert counts.sum() == n
+    # standalone histogram kernel on the same outputs, and on escape times with under/overflow
+    c2 = fpt.histogram(torch.from_numpy(g).cuda(), torch.from_numpy(s).cuda(), lo, hi, nb)
+    assert np.array_equal(_np(c2).astype(np.uint64), want)
+    c3 = fpt.histogram(torch.from_numpy(f).cuda(), None, 960.0, 990.0, 7)
+    assert np.array_equal(_np(c3).astype(np.uint64), oracle.histogram(f, None, 960.0, 990.0, 7))
+
+
+def test_config4_family_fp32_short_twin():
+    w = fpt.workload("c4", nu=1e-5, t_max=0.55 / 1e-5)                # same parameters, faster ramp: ~9e5 steps per path
+    n = 700
+    gpu = run_gpu(w, n)
+    ora = run_oracle(w, n)
+    assert_parity(gpu, ora, w["params"]["dt"], REL_FP32)
+    assert np.all(gpu[2] == 0)
+
+
+def test_config5_family_imbalanced():
+    w = fpt.workload("c5", temperature=0.08, t_max=4000 * 5e-3 * 100)   # mean ~1e5 steps, cap 4e5 steps: a few % censored
+    n = 3000
+    gpu = run_gpu(w, n)
+    ora = run_oracle(w, n)
+    assert_parity(gpu, ora, w["params"]["dt"], REL_FP64)
+    ncens = int(np.sum(ora["status"] == 1))
+    assert 0 < ncens < n // 2
+    assert fpt.last_stats()["n_censored"] == ncens
+    w2 = fpt.workload("c5", temperature=0.2)
+    f, g, s = run_gpu(w2, 4)
+    assert [int(round(t / 5e-3)) for t in f] == [5625, 11381, 16955, 21480]
+
+
+def test_all_other_kernel_variants_match():
+    """Every (model, scheme, amp, ramp, precision) instantiation at least once, ragged sizes."""
+    base = dict(alpha=0.3, temperature=0.2, gamma0=0.8, phi0=0.5, v0=0.0, threshold=4.0, dt=0.02)
+    for precision in ("fp64", "fp32"):
+        for model in ("overdamped", "underdamped"):
+            for scheme in ("em", "heun"):
+                for amp in (0.0, 1.0):
+                    for nu in (0.0, 2e-3):
+                        kw = dict(base, precision=precision, model=model, scheme=scheme, amp=amp, nu=nu)
+                        w = dict(params=kw, seed=21, t_max=40.0, n_traj=333)
+                        gpu = run_gpu(w)
+                        ora = run_oracle(w, 333)
+                        assert_parity(gpu, ora, kw["dt"], REL_FP64 if precision == "fp64" else REL_FP32)
+
+
+# P8: invariance
+def test_results_do_not_depend_on_K_geometry_or_sharding():
+    w = fpt.workload("c2", t_max=60.0)                                   # cap 6000 steps: a mix of escaped and censored
+    n = 4099
+    ref = run_gpu(w, n)
+    assert 0 < np.sum(ref[2] == 1) < n
+    for K in (1, 2, 6, 50, 64, 1000):
+        out = run_gpu(w, n, check_every=K)
+        assert all(np.array_equal(a, b) for a, b in zip(out, ref)), K
+    for geom in [(32, 1, 1), (32, 1, 3), (256, 1, 0), (96, 2, 0), (128, 0, 5)]:
+        fpt.set_launch(*geom)
+        try:
+            out = run_gpu(w, n)
+        finally:
+            fpt.set_launch(0, 0, 0)
+        assert all(np.array_equal(a, b) for a, b in zip(out, ref)), geom
+    a = run_gpu(w, 1000, first_id=0)
+    b = run_gpu(w, n - 1000, first_id=1000)
+    for i in range(3):
+        assert np.array_equal(np.concatenate([a[i], b[i]]), ref[i])
+    # fp32 path: K rounded to multiples of 4
+    w4 = fpt.workload("c4", nu=1e-4, t_max=0.55 / 1e-4)
+    r4 = run_gpu(w4, 257)
+    for K in (1, 5, 64):
+        out = run_gpu(w4, 257, check_every=K)
+        assert all(np.array_equal(x, y) for x, y in zip(out, r4)), K
+
+
+# edge and degenerate cases
+def test_edge_cases():
+    w = fpt.workload("c2")
+    p = fpt.make_params(**w["params"])
+    # empty input
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    fpt.simulate(p, 0, 1, 1.0, out=(e, e, torch.empty(0, dtype=torch.int32, device="cuda")))
+    # a single trajectory; gamma output omitted
+    f = torch.empty(1, dtype=torch.float64, device="cuda")
+    s = torch.empty(1, dtype=torch.int32, device="cuda")
+    fpt.simulate(p, 1, 2, w["t_max"], out=(f, None, s))
+    torch.cuda.synchronize()
+    assert int(round(float(f[0]) / 0.01)) == 9508 and int(s[0]) == 0
+    # caps that fall inside a poll interval, odd caps, cap of one step
+    for n_cap in (1, 2, 3, 15, 16, 17, 33, 9507, 9508, 9509):
+        ww = fpt.workload("c2", t_max=n_cap * 0.01)
+        gpu = run_gpu(ww, 64)
+        ora = run_oracle(ww, 64)
+        assert oracle.n_cap(oracle.make_params(**ww["params"]), ww["t_max"]) == n_cap
+        assert_parity(gpu, ora, 0.01, REL_FP64)
+        assert fpt.last_stats()["n_cap"] == n_cap
+    # initial state already beyond the threshold: escaped at k = 0
+    ww = fpt.workload("c2", threshold=1.0)
+    gpu = run_gpu(ww, 100)
+    assert np.all(gpu[0] == 0.0) and np.all(gpu[2] == 0) and np.all(gpu[1] == 0.9)
+    assert_parity(gpu, run_oracle(ww, 100), 0.01, REL_FP64)
+    # zero temperature below the critical bias: nothing ever escapes (all censored, paper's -1 sentinel)
+    ww = fpt.workload("c2", temperature=0.0, t_max=30.0)
+    gpu = run_gpu(ww, 100)
+    assert np.all(gpu[0] == -1.0) and np.all(gpu[2] == 1)
+    assert_parity(gpu, run_oracle(ww, 100), 0.01, REL_FP64)
+    # zero temperature above it: deterministic escape, every trajectory identical
+    ww = fpt.workload("c2", temperature=0.0, gamma0=1.2, phi0=0.0, threshold=2 * math.pi, alpha=0.1)
+    gpu = run_gpu(ww, 70)
+    assert np.all(gpu[2] == 0) and len(set(gpu[0].tolist())) == 1 and int(round(gpu[0][0] / 0.01)) == 430   # golden/deterministic.txt
+    # states that overflow: +inf crosses (escaped), -inf makes sin(phi) NaN (status 2, NaN outputs) -- same as the oracle
+    for prec, big in (("fp64", 1e300), ("fp32", 1e30)):
+        ww = dict(params=dict(model="overdamped", scheme="em", precision=prec, alpha=0.0, temperature=big, amp=1.0, gamma0=0.0,
+                              nu=0.0, phi0=0.0, v0=0.0, threshold=1e10, dt=big), seed=3, t_max=big * 100, n_traj=64)
+        gpu = run_gpu(ww)
+        ora = run_oracle(ww, 64)
+        assert np.array_equal(gpu[2], ora["status"]) and np.any(ora["status"] == 2) and np.any(ora["status"] == 0)
+        bad = ora["status"] == 2
+        assert np.all(np.isnan(gpu[0][bad])) and np.all(np.isnan(gpu[1][bad]))
+        assert np.array_equal(gpu[0][~bad], ora["fpt"][~bad])
+        assert fpt.last_stats()["n_nan"] == int(bad.sum())
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    w = fpt.workload("c3", nu=1e-3, t_max=1.05 / 1e-3)
+    n = 300
+    of, lo, hi, nb = w["hist"]
+    f, g, s, c = run_gpu(w, n, hist=True)
+    hf = torch.empty(n, dtype=torch.float64).pin_memory()
+    hg = torch.empty(n, dtype=torch.float64).pin_memory()
+    hs = torch.empty(n, dtype=torch.int32).pin_memory()
+    hc = np.zeros(nb + 2, dtype=np.uint64)
+    fpt.simulate_host(fpt.make_params(**w["params"]), n, w["seed"], w["t_max"], hf, hg, hs, hist=(of, lo, hi, nb, hc))
+    assert np.array_equal(hf.numpy(), f) and np.array_equal(hg.numpy(), g) and np.array_equal(hs.numpy(), s)
+    assert np.array_equal(hc, c)
+    hf2 = np.empty(n)
+    hs2 = np.empty(n, dtype=np.int32)
+    fpt.simulate_host(fpt.make_params(**w["params"]), n, w["seed"], w["t_max"], hf2, None, hs2)          # pageable, no gamma
+    assert np.array_equal(hf2, f) and np.array_equal(hs2, s)
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# full sizes, in the launch configuration bench.py times (default geometry): sampled ids against the oracle, plus
+# properties that hold at any size
+def test_config2_full_size_sampled():
+    w = fpt.workload("c2")
+    n = w["n_traj"]
+    f, g, s = run_gpu(w)
+    stats = fpt.last_stats()
+    assert stats["n_traj"] == n and stats["n_escaped"] + stats["n_censored"] + stats["n_nan"] == n
+    k = np.rint(f / 0.01).astype(np.int64)
+    assert np.all(s == 0) and stats["useful_steps"] == int(k.sum())
+    assert np.all(g == 0.9)
+    rng = np.random.default_rng(0)
+    for i in np.concatenate([rng.integers(0, n, 300), [0, n - 1, n - 2]]):
+        o = run_oracle(w, 1, first_id=int(i))
+        assert int(o["k"][0]) == int(k[i]) and o["fpt"][0] == f[i]
+    assert abs(k.mean() - 5690) < 5 * 4600 / math.sqrt(n) + 60           # SURVEY P7 probe: mean k_esc 5690 (independent numpy sample)
+    # distribution: GPU ids [0, 4000) against an independent oracle sample (other ids), two-sample KS
+    from scipy import stats as sst
+    ind = run_oracle(w, 4000, first_id=10**7)
+    assert sst.ks_2samp(f[:4000], ind["fpt"]).pvalue > 0.01
+
+
+def test_config1_distribution_vs_inverse_gaussian():
+    """GPU sample of config 1 against the closed form the oracle is pinned to (BGK-shifted inverse Gaussian)."""
+    from scipy import stats as sst
+    w = fpt.workload("c1", first_id=5 * 10**6)
+    f, g, s = run_gpu(w, 20000)
+    mu, D, dt = 1.0, 0.1, 1e-3
+    a = 1.0 + 0.5826 * math.sqrt(2 * D * dt)
+    lam = a * a / (2 * D)
+    cdf = lambda t: sst.invgauss.cdf(t, mu=(a / mu) / lam, scale=lam)
+    assert sst.kstest(f, cdf).pvalue > 0.01
+    assert abs(f.mean() - a / mu) < 5 * math.sqrt(0.2 / 20000)

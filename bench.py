@@ -1,0 +1,323 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the first-passage-time hot path (BASELINE.json metric: trajectory-steps/s and escapes/s on
+one B200, fraction of the FP64 pipe peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--impl ours|reference] [--no-extra]
+
+A "step" is one pass of the whole hot path (claim ids -> Philox -> Box-Muller -> integrate -> escape test -> refill ->
+results by id) over one batch: BASELINE.json configs[1] (C2: RCSJ constant bias, stochastic Heun, fp64, 10^5
+trajectories, seed 2), i.e. ONE fpt_simulate call.  Inputs are generated inside the kernel from (seed, trajectory id), so
+there are no input arrays; outputs (20 B per trajectory) stay in HBM for `value` and are copied to pinned host memory for
+`e2e` (fpt_simulate_host).  L2 is flushed between timed steps.  With N > 1 (torchrun) every rank integrates its own
+10^5-trajectory id range (first_id = rank * n_traj; no data-path collective): weak scaling.
+
+`--impl reference` times the ORACLE (oracle/fpt_oracle.cpp, OpenMP over trajectories) on the host cores, each step a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "trajectory-steps/s"
+UNIT = "steps/s"
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE persistent-kernel launch of the bench workload (C2, 10^5 trajectories),
+# from the `ncu --set full` capture summarised in profiles/r01_c2_full.md; None until that capture exists.
+NCU_DRAM_BYTES_PER_LAUNCH = None
+
+
+# ------------------------------------------------------------------------------------------------------------------
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    BAD = {"hw_slowdown": 0x8, "hw_thermal_slowdown": 0x40, "sw_thermal_slowdown": 0x20}
+    NOTE = {"sw_power_cap": 0x4}
+
+    def __init__(self, index: int, period_s: float = 0.01):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        while self.ok and not self._stop_evt.is_set():
+            try:
+                self.samples.append(float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                r = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for name, bit in {**self.BAD, **self.NOTE}.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_rate(w: dict, budget_s: float, n_max: int, first_id: int = 0):
+    """Time the oracle (all host cores) on the first ids of workload `w`; returns (steps/s, escapes/s, ids, seconds, cores)."""
+    import numpy as np
+    import oracle
+    p = oracle.make_params(**dict(w["params"], first_id=first_id))
+    cores = oracle.omp_threads()
+    n0 = min(n_max, 64 * cores)
+    t0 = time.perf_counter()
+    r = oracle.simulate(p, n0, w["seed"], w["t_max"])
+    dt0 = time.perf_counter() - t0
+    n = int(min(n_max, max(n0, n0 * budget_s / max(dt0, 1e-3))))
+    if n > n0 * 1.5:
+        t0 = time.perf_counter()
+        r = oracle.simulate(p, n, w["seed"], w["t_max"])
+        dt0 = time.perf_counter() - t0
+    else:
+        n = n0
+    steps = float(np.sum(r["k"]))
+    return steps / dt0, float(np.sum(r["status"] == 0)) / dt0, n, dt0, cores
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import paper_1802_05065_b200 as fpt
+    w = fpt.workload(args.workload)
+    per_step_budget = max(1.0, min(15.0, 90.0 / max(1, args.steps + args.warmup)))
+    rates, esc, ids, secs = [], [], 0, 0.0
+    cores = host_cores()
+    for i in range(args.warmup + args.steps):
+        r, e, n, dt, cores = oracle_rate(w, per_step_budget, w["n_traj"], first_id=0)
+        if i >= args.warmup:
+            rates.append(r); esc.append(e); ids = n; secs += dt
+    value = statistics.mean(rates)
+    sample = f"ids [0,{ids}) of {w['n_traj']} per step, OpenMP over trajectories, {cores} threads"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64" if w["params"]["precision"] == "fp64" else "f32", "data": "synthetic",
+            "config": {"workload": args.workload, "n_traj_per_step": ids},
+            "escapes_per_s": statistics.mean(esc),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+def time_workload(fpt, torch, w, n_traj, steps, warmup, flush, first_id=0, hist=False):
+    """Device-timed steps of one workload; returns dict(ms list, stats of the last step, outputs)."""
+    p = fpt.make_params(**dict(w["params"], first_id=first_id))
+    out = fpt.binding._alloc_outputs(n_traj)
+    counts = None
+    if hist and w.get("hist"):
+        of, lo, hi, nb = w["hist"]
+        counts = torch.zeros(nb + 2, dtype=torch.int64, device="cuda")
+
+    def one():
+        if counts is not None:
+            fpt.simulate_hist(p, n_traj, w["seed"], w["t_max"], lo, hi, nb, hist_of=of, counts=counts, out=out)
+        else:
+            fpt.simulate(p, n_traj, w["seed"], w["t_max"], out=out)
+
+    for _ in range(warmup):
+        one()
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(steps):
+        if flush is not None:
+            flush.add_(1)                       # write a buffer larger than L2 between timed steps
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        one()
+        e1.record()
+        e1.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    return {"ms": ms, "stats": fpt.last_stats(), "out": out}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--n-traj", type=int, default=0, help="override the trajectories per step (0 = the config's own count)")
+    ap.add_argument("--no-extra", action="store_true", help="skip the throughput-shaped extra workloads and the CPU baseline")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    import paper_1802_05065_b200 as fpt
+    fpt.lib()                                    # fails loudly if the CUDA extension is missing
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    w = fpt.workload(args.workload)
+    n_traj = w["n_traj"]
+    if args.workload in ("c3", "c4", "c5"):       # full configs take minutes: bench them on a fixed id range
+        n_traj = min(n_traj, 1 << 16)
+    if args.n_traj > 0:
+        n_traj = args.n_traj
+    n64 = w["n64_ref"]
+    fp32 = w["params"]["precision"] == "fp32"
+    flush = torch.zeros(256 << 20, dtype=torch.uint8, device="cuda")     # 256 MiB > 126 MB L2
+
+    # roofline denominator, measured live under ~1 s of load: FP64 (FP32 for the fp32 variant) thread-instructions / s
+    peak, clk_hz = (fpt.fp32_peak if fp32 else fpt.fp64_peak)(1.0)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-timed region: exactly K steps
+    first_id = rank * n_traj
+    time_workload(fpt, torch, w, n_traj, 0, args.warmup, flush, first_id)          # warm-up
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    t_wall0 = time.perf_counter()
+    res = time_workload(fpt, torch, w, n_traj, args.steps, 0, flush, first_id)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    st = res["stats"]
+    dev_s = sum(res["ms"]) * 1e-3
+    f, g, s = res["out"]
+    k = torch.where(s == 0, torch.round(f / w["params"]["dt"]), torch.full_like(f, float(st["n_cap"]))).to(torch.int64)
+    useful = int(k.sum().item())
+    assert useful == st["useful_steps"], (useful, st["useful_steps"])               # counters agree with the outputs
+    escaped = int((s == 0).sum().item())
+
+    # ---- end to end through the public host-buffer call (pinned host outputs, D2H inside the timed region)
+    hf = torch.empty(n_traj, dtype=torch.float64).pin_memory()
+    hg = torch.empty(n_traj, dtype=torch.float64).pin_memory()
+    hs = torch.empty(n_traj, dtype=torch.int32).pin_memory()
+    p_host = fpt.make_params(**dict(w["params"], first_id=first_id))
+    for _ in range(2):
+        fpt.simulate_host(p_host, n_traj, w["seed"], w["t_max"], hf, hg, hs)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        fpt.simulate_host(p_host, n_traj, w["seed"], w["t_max"], hf, hg, hs)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    assert torch.equal(hf, f.cpu()) and torch.equal(hs, s.cpu())
+
+    # ---- max over ranks
+    tv = torch.tensor([dev_s, e2e_s], dtype=torch.float64, device="cuda")
+    tot = torch.tensor([float(useful), float(escaped)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tv, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    dev_s, e2e_s = float(tv[0]), float(tv[1])
+    useful_all, escaped_all = float(tot[0]), float(tot[1])
+    value = useful_all * args.steps / dev_s
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32" if fp32 else "f64", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: BASELINE.json configs[{int(args.workload[1]) - 1}]", "n_traj_per_gpu": n_traj,
+                   "seed": w["seed"], "t_max": w["t_max"], "params": {k2: v for k2, v in w["params"].items()},
+                   "l2": "no input arrays (inputs are generated in-kernel from seed and id); 256 MiB written between timed steps",
+                   "parallelism": f"independent id ranges x{world}, no collective"},
+        "escapes_per_s": escaped_all * args.steps / dev_s,
+        "censored": int(st["n_censored"]), "lane_efficiency": st["lane_efficiency"],
+        "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"]},
+        "wall_s_timed_region": t_wall,
+        "e2e": {"value": useful_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 96,
+                "d2h_bytes_per_step": n_traj * 20, "api": "fpt_simulate_host (pinned host outputs; inputs = 96-byte fpt_params)"},
+        "gpu_launches": args.steps,             # one persistent-kernel launch per step (plus a memset and a 64-byte D2D copy)
+        "clocks": clocks,
+    }
+    per_gpu_rate = (useful * args.steps / (sum(res["ms"]) * 1e-3))
+    line["roofline"] = {
+        "bound": "alu", "achieved": per_gpu_rate * n64 / 1e9, "peak": peak / 1e9,
+        "unit": "G FP32 thread-instr/s" if fp32 else "G FP64 thread-instr/s",
+        "frac": per_gpu_rate * n64 / peak, "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+        "note": f"achieved = steps/s x {n64} reference {'FP32' if fp32 else 'FP64'}-pipe instructions per step (SURVEY 8(a)); peak = "
+                f"{'FFMA' if fp32 else 'DFMA'} chains measured live by fpt_fp{'32' if fp32 else '64'}_peak after 1 s of load "
+                f"(SM clock seen {clk_hz / 1e6:.0f} MHz); MEASURED_PEAKS.json has no {'FP32' if fp32 else 'FP64'} figure",
+        "hbm_bytes_per_step_algorithmic": n_traj * 20,
+    }
+
+    if rank == 0 and world == 1 and not args.no_extra:
+        # ---- throughput-shaped workloads (same parameters as the configs, id ranges sized to fill the GPU for ~0.1-1 s)
+        extra = {}
+        shapes = [("c2_x42", "c2", dict(), 1 << 22, False),
+                  ("c3_fast_ramp", "c3", dict(nu=1e-3, t_max=1050.0), 1 << 19, True),
+                  ("c5_T0.1", "c5", dict(temperature=0.1, t_max=2000.0), 1 << 20, False),
+                  ("c4_fast_ramp", "c4", dict(nu=1e-4, t_max=5500.0), 1 << 18, False)]
+        for name, base, ov, n, hist in shapes:
+            ww = fpt.workload(base, **ov)
+            r = time_workload(fpt, torch, ww, n, 3, 1, flush, 0, hist=hist)
+            sec = statistics.median(r["ms"]) * 1e-3
+            stx = r["stats"]
+            is32 = ww["params"]["precision"] == "fp32"
+            pk = peak if is32 == fp32 else (fpt.fp32_peak if is32 else fpt.fp64_peak)(0.5)[0]
+            extra[name] = {"n_traj": n, "overrides": ov, "steps_per_s": stx["useful_steps"] / sec, "escapes_per_s": stx["n_escaped"] / sec,
+                           "ms": sec * 1e3, "censored": stx["n_censored"], "lane_efficiency": stx["lane_efficiency"],
+                           "roofline_frac": stx["useful_steps"] / sec * ww["n64_ref"] / pk, "n_ref_per_step": ww["n64_ref"],
+                           "dtype": "f32" if is32 else "f64"}
+        line["extra_workloads"] = extra
+        # ---- the oracle as it stands on the host cores, bounded sample of the same workload
+        r_cpu, e_cpu, ids, secs, cores = oracle_rate(w, 15.0, n_traj)
+        line["cpu_baseline"] = {"value": r_cpu, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"ids [0,{ids}) of the bench workload, {secs:.1f} s, OpenMP over trajectories",
+                                "escapes_per_s": e_cpu}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -245,9 +245,16 @@ __global__ void fpt_histogram_kernel(const double* __restrict__ values, const in
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// Roofline denominators: independent fma chains, 8 per thread, every SM full.
+// Roofline denominators: independent fma chains, 8 per thread, every SM full.  The SM clock is read from clock64 (a
+// per-SM counter): every block records its start and end into its SM's slot, the host takes the longest span.
+constexpr int kMaxSm = 256;
+struct PeakClocks {
+  long long t_min[kMaxSm];
+  long long t_max[kMaxSm];
+};
+
 template <typename T>
-__global__ void __launch_bounds__(256) fpt_peak_kernel(T* sink, int iters, long long* clocks) {
+__global__ void __launch_bounds__(256) fpt_peak_kernel(T* sink, int iters, PeakClocks* clk) {
   T a[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) a[i] = (T)(threadIdx.x + i) * (T)1e-3;
@@ -268,7 +275,14 @@ __global__ void __launch_bounds__(256) fpt_peak_kernel(T* sink, int iters, long 
 #pragma unroll
   for (int i = 0; i < 8; ++i) s += a[i];
   if (s == (T)123456.789) sink[0] = s;
-  if (threadIdx.x == 0 && blockIdx.x == 0) clocks[0] = t1 - t0;
+  if (threadIdx.x == 0) {
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    if (smid < (unsigned)kMaxSm) {
+      atomicMin(&clk->t_min[smid], t0);
+      atomicMax(&clk->t_max[smid], t1);
+    }
+  }
 }
 
 template <typename T>
@@ -278,47 +292,43 @@ int peak_impl(double seconds, double* inst_per_s, double* sm_clock_hz) {
   int rc = device_ctx(&ctx);
   if (rc != FPT_OK) return rc;
   T* sink = nullptr;
-  long long* d_clk = nullptr;
+  PeakClocks* d_clk = nullptr;
   FPT_CUDA(cudaMalloc(&sink, sizeof(T)));
-  FPT_CUDA(cudaMalloc(&d_clk, sizeof(long long)));
+  FPT_CUDA(cudaMalloc(&d_clk, sizeof(PeakClocks)));
   cudaEvent_t e0, e1;
   FPT_CUDA(cudaEventCreate(&e0));
   FPT_CUDA(cudaEventCreate(&e1));
-  const int block = 256, grid = ctx->sm_count * 8;
+  const int block = 256, grid = ctx->sm_count * 8;            // 2048 threads per SM, one wave
   const int iters = sizeof(T) == 8 ? 4096 : 16384;
   const double inst_per_launch = (double)grid * block * (double)iters * 64.0;
+  std::vector<long long> h(2 * kMaxSm);
+  auto reset_clk = [&]() {
+    for (int i = 0; i < kMaxSm; ++i) { h[i] = 0x7fffffffffffffffll; h[kMaxSm + i] = 0; }
+    return cudaMemcpy(d_clk, h.data(), sizeof(PeakClocks), cudaMemcpyHostToDevice);
+  };
+  FPT_CUDA(reset_clk());
   fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);   // warm-up
   FPT_CUDA(cudaDeviceSynchronize());
-  double best = 0.0, total_ms = 0.0, clk_hz = 0.0;
+  double total_ms = 0.0;
+  float ms = 0.f;
   int launches = 0;
-  while (total_ms < seconds * 1e3 && launches < 100000) {
+  // load the GPU for `seconds`, then report the LAST launch: the sustained rate and clock under this load
+  do {
+    FPT_CUDA(reset_clk());
     FPT_CUDA(cudaEventRecord(e0));
     fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);
     FPT_CUDA(cudaEventRecord(e1));
     FPT_CUDA(cudaEventSynchronize(e1));
-    float ms = 0.f;
     FPT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
     total_ms += ms;
     ++launches;
-    const double rate = inst_per_launch / (ms * 1e-3);
-    if (rate > best) best = rate;
-  }
-  // sustained figure: the LAST launch (after `seconds` of load), and the clock of block 0 of a single-wave launch
-  {
-    FPT_CUDA(cudaEventRecord(e0));
-    fpt_peak_kernel<T><<<grid, block>>>(sink, iters, d_clk);
-    FPT_CUDA(cudaEventRecord(e1));
-    FPT_CUDA(cudaEventSynchronize(e1));
-    float ms = 0.f;
-    FPT_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-    long long clk = 0;
-    FPT_CUDA(cudaMemcpy(&clk, d_clk, sizeof(clk), cudaMemcpyDeviceToHost));
-    // all 8 blocks/SM are co-resident (256 thr x 8 = 2048), so block 0 runs for the whole launch
-    clk_hz = (double)clk / (ms * 1e-3);
-    *inst_per_s = inst_per_launch / (ms * 1e-3);
-  }
-  if (sm_clock_hz) *sm_clock_hz = clk_hz;
-  (void)best;
+  } while (total_ms < seconds * 1e3 && launches < 100000);
+  *inst_per_s = inst_per_launch / (ms * 1e-3);
+  FPT_CUDA(cudaMemcpy(h.data(), d_clk, sizeof(PeakClocks), cudaMemcpyDeviceToHost));
+  long long span = 0;
+  for (int i = 0; i < kMaxSm; ++i)
+    if (h[kMaxSm + i] > h[i]) span = std::max(span, h[kMaxSm + i] - h[i]);
+  if (sm_clock_hz) *sm_clock_hz = (double)span / (ms * 1e-3);
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   cudaFree(sink);

@@ -146,6 +146,11 @@ int fpt_dbg_unary_f32(int32_t which, const float* x, float* y, int64_t n, void* 
 /* cos, sin of the Box-Muller angle from the raw 64-bit (fp64) / 32-bit (fp32) word */
 int fpt_dbg_sincos_f64(const uint64_t* Y, double* c, double* s, int64_t n, void* cuda_stream);
 int fpt_dbg_sincos_f32(const uint32_t* o, float* c, float* s, int64_t n, void* cuda_stream);
+/* the guard-free division / square-root sequences of csrc/fpt_math.cuh against nvcc's IEEE builtins, on operands drawn
+ * from the real pipeline (n_threads streams, a multiple of 128, x blocks_per_thread Philox blocks each):
+ * out4[0..3] += number of bit mismatches {fp64 div, fp64 sqrt, fp32 div, fp32 sqrt} (device, uint64, caller zeroes). */
+int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t blocks_per_thread, uint64_t* out4,
+                      void* cuda_stream);
 /* one trajectory (id) with its states recorded: trace_phi[k], trace_v[k] for k = 0..min(k_end, trace_len-1) (as double),
  * out_status[0], out_k_end[0]; entries past k_end are left untouched. */
 int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len,

@@ -65,6 +65,7 @@ _SIGNATURES = {
     "fpt_dbg_unary_f32": [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
     "fpt_dbg_sincos_f64": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
     "fpt_dbg_sincos_f32": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
+    "fpt_dbg_selfcheck": [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_dbg_trace": [C.POINTER(FptParams), C.c_uint64, C.c_uint64, C.c_double, C.c_int64, C.c_void_p, C.c_void_p,
                       C.c_void_p, C.c_void_p, C.c_void_p],
 }
@@ -242,6 +243,13 @@ def dbg_sincos_f32(o, stream=None):
     s = torch.empty_like(c)
     _check(lib().fpt_dbg_sincos_f32(_ptr(o), _ptr(c), _ptr(s), o.numel(), _stream(stream)), "fpt_dbg_sincos_f32")
     return c, s
+
+
+def dbg_selfcheck(seed, id0, n_threads, blocks_per_thread, stream=None):
+    import torch
+    out = torch.zeros(4, dtype=torch.int64, device="cuda")
+    _check(lib().fpt_dbg_selfcheck(seed, id0, n_threads, blocks_per_thread, _ptr(out), _stream(stream)), "fpt_dbg_selfcheck")
+    return out
 
 
 def dbg_trace(params: FptParams, seed, tid, t_max, trace_len, stream=None):

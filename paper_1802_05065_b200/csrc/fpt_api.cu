@@ -392,6 +392,47 @@ __global__ void dbg_sincos32_kernel(const uint32_t* o, float* c, float* s, long 
   c[i] = cc; s[i] = ss;
 }
 
+// guard-free division / square root against nvcc's builtins on operands drawn from the real pipeline
+// (Philox block -> u1 -> m -> (m-1)/(m+1); w = -2 ln u1 -> sqrt w), fp64 and fp32: out[0..3] = mismatch counts
+__global__ void dbg_selfcheck_kernel(PhiloxKeys K, unsigned long long id0, int blocks_per_thread, unsigned long long* out) {
+  const unsigned long long id = id0 + (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned bad_div = 0, bad_sqrt = 0, bad_divf = 0, bad_sqrtf = 0;
+  for (int b = 0; b < blocks_per_thread; ++b) {
+    uint32_t o0, o1, o2, o3;
+    philox_block(K, (uint32_t)b, 0u, (uint32_t)id, (uint32_t)(id >> 32), o0, o1, o2, o3);
+    {
+      const double d = __hiloint2double((int)(0x3FF00000u | (o0 >> 12)), (int)__funnelshift_r(o1, o0, 12));
+      const double u1 = __dadd_rn(__dadd_rn(d, -1.0), 0x1p-53);
+      const uint32_t hi2 = (uint32_t)__double2hiint(u1) + (0x3FF00000u - 0x3FE6A09Eu);
+      const double m = __hiloint2double((int)((hi2 & 0x000FFFFFu) + 0x3FE6A09Eu), __double2loint(u1));
+      const double a = __dadd_rn(m, -1.0), bb = __dadd_rn(m, 1.0);
+      if (__double_as_longlong(div_rn_inrange(a, bb)) != __double_as_longlong(__ddiv_rn(a, bb))) ++bad_div;
+      const double w = neg2log(u1);
+      if (__double_as_longlong(sqrt_rn_inrange(w)) != __double_as_longlong(__dsqrt_rn(w))) ++bad_sqrt;
+      // a second, denser family: w straight from the random bits, spread over [2^-52, 128)
+      const double w2 = __hiloint2double((int)(0x3CB00000u + (o2 % 0x03B00000u)), (int)o3);
+      if (__double_as_longlong(sqrt_rn_inrange(w2)) != __double_as_longlong(__dsqrt_rn(w2))) ++bad_sqrt;
+    }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const uint32_t o = h ? o2 : o0;
+      const float u1 = __fmaf_rn(__uint2float_rn(o), 0x1p-32f, 0x1p-33f);
+      const uint32_t ix2 = (uint32_t)__float_as_int(u1) + (0x3f800000u - 0x3f3504f3u);
+      const float m = __int_as_float((int)((ix2 & 0x007fffffu) + 0x3f3504f3u));
+      const float a = __fadd_rn(m, -1.0f), bb = __fadd_rn(m, 1.0f);
+      if (__float_as_int(div_rn_inrange_f(a, bb)) != __float_as_int(__fdiv_rn(a, bb))) ++bad_divf;
+      const float w = neg2log_f(u1);
+      if (__float_as_int(sqrt_rn_inrange_f(w)) != __float_as_int(__fsqrt_rn(w))) ++bad_sqrtf;
+      const float w2 = __int_as_float((int)(0x33000000u + ((h ? o3 : o1) % 0x10000000u)));      // [2^-25, 2^7)
+      if (__float_as_int(sqrt_rn_inrange_f(w2)) != __float_as_int(__fsqrt_rn(w2))) ++bad_sqrtf;
+    }
+  }
+  if (bad_div) atomicAdd(&out[0], (unsigned long long)bad_div);
+  if (bad_sqrt) atomicAdd(&out[1], (unsigned long long)bad_sqrt);
+  if (bad_divf) atomicAdd(&out[2], (unsigned long long)bad_divf);
+  if (bad_sqrtf) atomicAdd(&out[3], (unsigned long long)bad_sqrtf);
+}
+
 inline int grid_for(long long n, int block) { return (int)((n + block - 1) / block); }
 
 }  // namespace
@@ -558,6 +599,14 @@ int fpt_dbg_sincos_f32(const uint32_t* o, float* c, float* sn, int64_t n, void* 
   if (!o || !c || !sn || n < 0) return FPT_E_INVALID;
   if (n == 0) return FPT_OK;
   dbg_sincos32_kernel<<<grid_for(n, 128), 128, 0, (cudaStream_t)s>>>(o, c, sn, n);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}
+int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t blocks_per_thread, uint64_t* out4, void* s) {
+  if (!out4 || n_threads < 0 || blocks_per_thread < 1 || (n_threads % 128) != 0) return FPT_E_INVALID;
+  if (n_threads == 0) return FPT_OK;
+  dbg_selfcheck_kernel<<<(int)(n_threads / 128), 128, 0, (cudaStream_t)s>>>(philox_round_keys(seed), id0, blocks_per_thread,
+                                                                          (unsigned long long*)out4);
   FPT_CUDA(cudaGetLastError());
   return FPT_OK;
 }

@@ -196,6 +196,11 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
   uint32_t id_lo = 0, id_hi = 0;
   unsigned long long s_useful = 0, s_blocks = 0;
   unsigned s_esc = 0, s_cens = 0, s_nan = 0, s_atom = 0;
+  // Software pipeline: zc holds the normals of the NEXT macro step to integrate; each loop iteration generates the
+  // normals of the one after it (Philox + Box-Muller, independent of the state) alongside the dependent step chain.
+  typename S::real zc[M];
+#pragma unroll
+  for (int s = 0; s < M; ++s) zc[s] = 0;
 
   for (;;) {
     // ---- S7 poll + S0 claim: idle lanes take new ids, one atomic per warp
@@ -220,6 +225,9 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
             kbase = 0;
             st.init(P);
             active = true;
+            uint32_t o0, o1, o2, o3;                              // normals of block 0 of the new stream
+            philox_block(P.keys, 0u, 0u, id_lo, id_hi, o0, o1, o2, o3);
+            S::normals(o0, o1, o2, o3, zc);
           }
         }
         exhausted = (base + cnt >= P.n_traj);
@@ -234,14 +242,14 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
     bool captured = false;
 #pragma unroll 1
     for (int jj = 0; jj < n_macro; ++jj) {
-      const unsigned long long b = b0 + (unsigned long long)jj;
+      const unsigned long long bn = b0 + (unsigned long long)(jj + 1);
       uint32_t o0, o1, o2, o3;
-      philox_block(P.keys, (uint32_t)b, (uint32_t)(b >> 32), id_lo, id_hi, o0, o1, o2, o3);
-      typename S::real z[M];
-      S::normals(o0, o1, o2, o3, z);
+      philox_block(P.keys, (uint32_t)bn, (uint32_t)(bn >> 32), id_lo, id_hi, o0, o1, o2, o3);
+      typename S::real zn[M];
+      S::normals(o0, o1, o2, o3, zn);
 #pragma unroll
       for (int s = 0; s < M; ++s) {
-        st.step(P, z[s]);
+        st.step(P, zc[s]);
         const bool hit = st.crossed(P) && !captured;      // sticky per-step test
         if (hit) {
           koff = jj * M + s + 1;
@@ -249,6 +257,8 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
         }
         captured = captured || hit;
       }
+#pragma unroll
+      for (int s = 0; s < M; ++s) zc[s] = zn[s];
     }
     ++s_blocks;
 

@@ -162,6 +162,14 @@ def test_elementary_functions_bit_exact():
     assert same_bits(_np(c), wc) and same_bits(_np(s), ws)
 
 
+def test_guard_free_div_sqrt_match_ieee_builtins():
+    """csrc/fpt_math.cuh replaces a/b and sqrt() by nvcc's fast-path sequences without the slow-path branch; on ~2e9
+    in-domain operands per function they must agree bit for bit with the IEEE builtins (so also with the oracle's / and sqrt)."""
+    bad = _np(fpt.dbg_selfcheck(12345, 0, 1 << 20, 1024))
+    torch.cuda.synchronize()
+    assert bad.tolist() == [0, 0, 0, 0], bad
+
+
 # states, step by step
 @pytest.mark.parametrize("precision", ["fp64", "fp32"])
 @pytest.mark.parametrize("model,scheme", [("overdamped", "em"), ("overdamped", "heun"), ("underdamped", "em"), ("underdamped", "heun")])

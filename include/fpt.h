@@ -82,6 +82,7 @@ typedef struct fpt_stats {
   int32_t  grid, block;        /* launch geometry used                                                    */
   int32_t  check_every;        /* effective K                                                             */
   int32_t  reserved;
+  uint64_t migrations;         /* trajectories parked by a sparse warp and adopted by another (drain-phase compaction) */
 } fpt_stats;
 
 /* Integrate trajectories id = first_id .. first_id+n_traj-1 until first passage or the cap n_cap = nearbyint(t_max/dt).

@@ -17,7 +17,7 @@ constexpr int kMaxFusedBins = 8192;
 struct DevStats {                 // device-side counters, one block of 8 x u64
   unsigned long long next_id;     // the global trajectory counter (S7)
   unsigned long long n_escaped, n_censored, n_nan;
-  unsigned long long useful_steps, issued_lane_steps, refill_atomics, pad;
+  unsigned long long useful_steps, issued_lane_steps, refill_atomics, migrations;
 };
 
 struct KParams {
@@ -35,6 +35,13 @@ struct KParams {
   unsigned long long* out_counts;
   DevStats* ws;
   PhiloxKeys keys;
+};
+
+// A trajectory parked between two polls (drain-phase lane compaction, see the persistent kernel): everything that is
+// not a pure function of (id, k).  The normals of the next macro step and the ramp registers are recomputed on adoption.
+struct ParkSlot {
+  unsigned long long a, b;        // fp64: bits of phi, v;  fp32: (phi, v) and the Kahan pair (t, c), two floats per word
+  unsigned long long kbase, idx;
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -73,21 +80,40 @@ struct State64 {
         const double f2 = force(P, phip, g2);
         phi = __fma_rn(P.sigma, z, __fma_rn(P.h2, __dadd_rn(f1, f2), phi));
       }
-    } else {
+    } else if (SCHEME == 0) {
       const double a1 = __fma_rn(-P.alpha, v, force(P, phi, g1));
       const double phip = __fma_rn(v, P.dt, phi);                              // both from the OLD state (Alg. 1 l. 11-12)
       const double vp = __fma_rn(P.sigma, z, __fma_rn(a1, P.dt, v));
-      if (SCHEME == 0) {
-        phi = phip;
-        v = vp;
-      } else {
-        const double a2 = __fma_rn(-P.alpha, vp, force(P, phip, g2));
-        phi = __fma_rn(P.h2, __dadd_rn(v, vp), phi);
-        v = __fma_rn(P.sigma, z, __fma_rn(P.h2, __dadd_rn(a1, a2), v));
+      phi = phip;
+      v = vp;
+    } else {
+      // Heun: the predictor phi_p does not depend on the first force, so both sines are evaluated side by side
+      const double phip = __fma_rn(v, P.dt, phi);
+      double f1 = g1, f2 = g2;
+      if (AMP) {
+        double s1, s2;
+        sin_drift2(phi, phip, s1, s2);
+        f1 = __fma_rn(-P.amp, s1, g1);
+        f2 = __fma_rn(-P.amp, s2, g2);
       }
+      const double a1 = __fma_rn(-P.alpha, v, f1);
+      const double vp = __fma_rn(P.sigma, z, __fma_rn(a1, P.dt, v));
+      const double a2 = __fma_rn(-P.alpha, vp, f2);
+      phi = __fma_rn(P.h2, __dadd_rn(v, vp), phi);
+      v = __fma_rn(P.sigma, z, __fma_rn(P.h2, __dadd_rn(a1, a2), v));
     }
   }
-  // re-synchronise the fp counter after the lane was given a fresh trajectory or at a poll (exact)
+  __device__ __forceinline__ void park(ParkSlot& s) const {
+    s.a = (unsigned long long)__double_as_longlong(phi);
+    s.b = (unsigned long long)__double_as_longlong(v);
+  }
+  // k is a poll boundary; kd and gamma_k are exact functions of k (the running g is always fma(dgamma, kd, gamma0))
+  __device__ __forceinline__ void unpark(const KParams& P, const ParkSlot& s, unsigned long long k) {
+    phi = __longlong_as_double((long long)s.a);
+    v = __longlong_as_double((long long)s.b);
+    kd = __ull2double_rn(k);
+    g = __fma_rn(P.dgamma, kd, P.gamma0);
+  }
   __device__ __forceinline__ bool crossed(const KParams& P) const { return !(phi < P.thr); }   // phi >= thr, or NaN
   __device__ __forceinline__ bool is_nan_hi(int hi) const { return ((unsigned)hi & 0x7fffffffu) > 0x7ff00000u; }
   __device__ __forceinline__ int phi_hi() const { return __double2hiint(phi); }
@@ -149,6 +175,16 @@ struct State32 {
       }
     }
   }
+  __device__ __forceinline__ void park(ParkSlot& s) const {
+    s.a = ((unsigned long long)(unsigned)__float_as_int(v) << 32) | (unsigned)__float_as_int(phi);
+    s.b = ((unsigned long long)(unsigned)__float_as_int(c) << 32) | (unsigned)__float_as_int(t);
+  }
+  __device__ __forceinline__ void unpark(const KParams&, const ParkSlot& s, unsigned long long) {
+    phi = __int_as_float((int)(unsigned)s.a);
+    v = __int_as_float((int)(unsigned)(s.a >> 32));
+    t = __int_as_float((int)(unsigned)s.b);
+    c = __int_as_float((int)(unsigned)(s.b >> 32));
+  }
   __device__ __forceinline__ bool crossed(const KParams& P) const { return !(phi < P.thr_f); }
   __device__ __forceinline__ bool is_nan_hi(int hi) const { return ((unsigned)hi & 0x7fffffffu) > 0x7f800000u; }
   __device__ __forceinline__ int phi_hi() const { return __float_as_int(phi); }
@@ -174,15 +210,54 @@ __device__ __forceinline__ int hist_slot(double x, double lo, double scale, int 
 // ---------------------------------------------------------------------------------------------------------------
 // The persistent kernel.  Grid = (#SM x resident blocks); each warp loops { poll+refill ; K steps } until the global
 // counter is exhausted and all of its lanes are idle.
+// Launch bounds steer ptxas' scheduler: with a minimum-blocks figure it assumes few resident warps and interleaves the
+// independent FP64 chains of a step (two Heun sines, the log / sin / cos polynomials of the next normals), which is
+// what a warp needs when it runs nearly alone (drain phase, under-filled configs); without one it serialises every
+// chain behind its 8-cycle DFMA latency and relies on other warps.
+#ifndef FPT_LB_THREADS
+#define FPT_LB_THREADS 256
+#endif
+#ifndef FPT_LB_MINBLOCKS
+#define FPT_LB_MINBLOCKS 1
+#endif
+constexpr int kMaxWarpsPerBlock = FPT_LB_THREADS / 32;
+
+// Drain-phase lane compaction (per block, shared memory).  Once the global id counter is exhausted a warp cannot refill
+// its finished lanes; without help it would keep issuing full-width instructions for its last few trajectories.  Here a
+// warp whose live lanes fit into the holes of the block's other warps PARKS them in `slots` and retires; warps with
+// holes ADOPT parked trajectories at their next poll.  Invariant (under `lock`): n_parked <= sum of holes[] over the
+// live warps that have seen exhaustion, so every parked trajectory is adopted and a warp that finds nothing left to do
+// may retire.  Results cannot change: a trajectory's state at a poll boundary is (phi, v[, t, c], k), everything else is
+// recomputed from (id, k).
+struct DrainPool {
+  int lock;
+  int n_parked;
+  int holes[kMaxWarpsPerBlock];
+  ParkSlot slots[FPT_LB_THREADS];
+};
+
+#if FPT_LB_MINBLOCKS > 0
+#define FPT_LAUNCH_BOUNDS __launch_bounds__(FPT_LB_THREADS, FPT_LB_MINBLOCKS)
+#else
+#define FPT_LAUNCH_BOUNDS __launch_bounds__(FPT_LB_THREADS)
+#endif
+
 template <class S>
-__global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_constant__ KParams P) {
+__global__ void FPT_LAUNCH_BOUNDS fpt_persistent_kernel(const __grid_constant__ KParams P) {
   extern __shared__ unsigned int smem_hist[];            // nbins + 2 counters when P.hist_of >= 0
+  __shared__ DrainPool pool;
   const bool do_hist = P.hist_of >= 0;
-  if (do_hist) {
+  if (do_hist)
     for (int i = threadIdx.x; i < P.nbins + 2; i += blockDim.x) smem_hist[i] = 0u;
-    __syncthreads();
+  if (threadIdx.x < kMaxWarpsPerBlock) pool.holes[threadIdx.x] = 0;
+  if (threadIdx.x == 0) {
+    pool.lock = 0;
+    pool.n_parked = 0;
   }
+  __syncthreads();
   const unsigned lane = threadIdx.x & 31u;
+  const int warp_in_block = (int)(threadIdx.x >> 5);
+  const int warps_in_block = (int)(blockDim.x >> 5);
   const unsigned lt_mask = (1u << lane) - 1u;
   constexpr int M = S::kMacro;
   const int n_macro = P.K / M;
@@ -195,7 +270,7 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
   unsigned long long kbase = 0;         // steps completed by the lane's trajectory at the last poll
   uint32_t id_lo = 0, id_hi = 0;
   unsigned long long s_useful = 0, s_blocks = 0;
-  unsigned s_esc = 0, s_cens = 0, s_nan = 0, s_atom = 0;
+  unsigned s_esc = 0, s_cens = 0, s_nan = 0, s_atom = 0, s_mig = 0;
   // Software pipeline: zc holds the normals of the NEXT macro step to integrate; each loop iteration generates the
   // normals of the one after it (Philox + Box-Muller, independent of the state) alongside the dependent step chain.
   typename S::real zc[M];
@@ -232,7 +307,71 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
         }
         exhausted = (base + cnt >= P.n_traj);
       }
-      if (__all_sync(0xffffffffu, !active)) break;
+      // ---- drain: lanes that could not be refilled adopt parked trajectories; a sparse warp parks its own and retires
+      const unsigned idle = __ballot_sync(0xffffffffu, !active);
+      if (idle) {                                           // implies exhausted
+        if (lane == 0)
+          while (atomicCAS(&pool.lock, 0, 1) != 0) __nanosleep(64);
+        __syncwarp();
+        __threadfence_block();
+        int np = *(volatile int*)&pool.n_parked;
+        int na = 32 - __popc(idle);
+        const int take = min(32 - na, np);
+        bool adopted = false;
+        if (!active) {
+          const int r = __popc(idle & lt_mask);
+          if (r < take) {
+            const ParkSlot sl = pool.slots[np - 1 - r];
+            idx = sl.idx;
+            kbase = sl.kbase;
+            st.unpark(P, sl, kbase);
+            active = true;
+            adopted = true;
+          }
+        }
+        np -= take;
+        na += take;
+        bool retire = (na == 0);                            // nothing of our own and (then necessarily) nothing parked
+        if (!retire && na < 32) {
+          int others = 0;
+          for (int w = 0; w < warps_in_block; ++w)
+            if (w != warp_in_block) others += *(volatile int*)&pool.holes[w];
+          if (na <= others - np) {                          // the other warps' holes can take all of ours
+            const unsigned live = __ballot_sync(0xffffffffu, active);
+            if (active) {
+              ParkSlot sl;
+              st.park(sl);
+              sl.kbase = kbase;
+              sl.idx = idx;
+              pool.slots[np + __popc(live & lt_mask)] = sl;
+              active = false;
+              adopted = false;
+              ++s_mig;
+            }
+            np += na;
+            retire = true;
+          }
+        }
+        __threadfence_block();
+        __syncwarp();
+        if (lane == 0) {
+          *(volatile int*)&pool.n_parked = np;
+          *(volatile int*)&pool.holes[warp_in_block] = retire ? 0 : 32 - na;
+          __threadfence_block();
+          atomicExch(&pool.lock, 0);
+        }
+        __syncwarp();
+        if (retire) break;
+        if (adopted) {                                      // stream position of the adopted trajectory: block kbase / M
+          const unsigned long long id = P.first_id + idx;
+          id_lo = (uint32_t)id;
+          id_hi = (uint32_t)(id >> 32);
+          const unsigned long long b = kbase / (unsigned long long)M;
+          uint32_t o0, o1, o2, o3;
+          philox_block(P.keys, (uint32_t)b, (uint32_t)(b >> 32), id_lo, id_hi, o0, o1, o2, o3);
+          S::normals(o0, o1, o2, o3, zc);
+        }
+      }
     }
 
     // ---- K steps (S1..S6).  Block index of macro step jj of this poll interval: kbase/M + jj.
@@ -312,6 +451,7 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
   const unsigned c = __reduce_add_sync(0xffffffffu, s_cens);
   const unsigned nn = __reduce_add_sync(0xffffffffu, s_nan);
   s_atom = __reduce_add_sync(0xffffffffu, s_atom);
+  s_mig = __reduce_add_sync(0xffffffffu, s_mig);
   if (lane == 0) {
     atomicAdd(&P.ws->useful_steps, s_useful);
     atomicAdd(&P.ws->issued_lane_steps, s_blocks * (unsigned long long)P.K * 32ull);
@@ -319,6 +459,7 @@ __global__ void __launch_bounds__(256) fpt_persistent_kernel(const __grid_consta
     atomicAdd(&P.ws->n_censored, (unsigned long long)c);
     atomicAdd(&P.ws->n_nan, (unsigned long long)nn);
     atomicAdd(&P.ws->refill_atomics, (unsigned long long)s_atom);
+    if (s_mig) atomicAdd(&P.ws->migrations, (unsigned long long)s_mig);
   }
   if (do_hist) {
     __syncthreads();

@@ -302,6 +302,34 @@ def test_results_do_not_depend_on_K_geometry_or_sharding():
         assert all(np.array_equal(x, y) for x, y in zip(out, r4)), K
 
 
+def test_drain_compaction_parks_and_adopts_without_changing_results():
+    """Drain phase (ids exhausted): sparse warps park their trajectories in shared memory and other warps of the block
+    adopt them.  A parked trajectory resumes from (phi, v[, t, c], k) with its Philox position, ramp registers and
+    Kahan pair rebuilt -- results must stay those of the oracle, for every state layout, and migrations must occur."""
+    cases = [
+        (fpt.workload("c2", t_max=300.0), 2048, REL_FP64),                                  # fp64 Heun underdamped, nu = 0
+        (fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3), 1024, REL_FP64),                   # fp64 ramp: kd, gamma_k rebuilt
+        (fpt.workload("c5", temperature=0.1, t_max=1500.0), 2048, REL_FP64),                # fp64 EM overdamped
+        (fpt.workload("c4", nu=2e-5, t_max=0.55 / 2e-5), 1024, REL_FP32),                   # fp32: Kahan pair carried
+        (dict(params=dict(model="overdamped", scheme="heun", precision="fp32", temperature=0.3, gamma0=0.6, phi0=0.5,
+                          threshold=5.0, dt=0.01, amp=1.0), seed=33, t_max=400.0), 1024, REL_FP32),
+    ]
+    for w, n, rel in cases:
+        fpt.set_launch(256, 1, n // 256)                 # every trajectory resident at once: the whole run is a drain
+        try:
+            gpu = run_gpu(w, n, check_every=8)
+            st = fpt.last_stats()
+        finally:
+            fpt.set_launch(0, 0, 0)
+        ora = run_oracle(w, n)
+        assert_parity(gpu, ora, w["params"]["dt"], rel)
+        assert st["useful_steps"] == int(np.sum(ora["k"]))
+        assert st["migrations"] > 0, "compaction never triggered"
+        # exponential-ish lengths: without compaction each warp lives as long as its slowest lane (efficiency ~ 1/H_32)
+        if w["params"].get("nu", 0.0) == 0.0:
+            assert st["lane_efficiency"] > 0.5, st
+
+
 # edge and degenerate cases
 def test_edge_cases():
     w = fpt.workload("c2")

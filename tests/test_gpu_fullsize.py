@@ -1,0 +1,110 @@
+"""Full-size runs of BASELINE.json configs 3, 4 and 5 (minutes to tens of minutes of GPU time each), once for the record.
+
+Skipped unless FPT_FULLSIZE names the configs to run, e.g.
+
+    FPT_FULLSIZE=c3,c5,c4 python -m pytest tests/test_gpu_fullsize.py -m gpu -x -q -s
+
+Each test runs the whole config through the C ABI in the library's default launch configuration, timed with CUDA
+events, and checks it against the oracle on SAMPLED trajectory ids (the oracle needs seconds to minutes per
+trajectory at these lengths, so it cannot do them all): status, escape step index, escape time and bias at escape must
+be bit-identical for every sampled id.  What holds at any size is checked on everything: counters against the outputs,
+histogram against the per-trajectory biases, value ranges.  The oracle runs on the host cores WHILE the kernel runs.
+A record with throughput, lane efficiency and the censored count is written to gpurun_out/fullsize_<config>.json.
+"""
+import json
+import os
+import time
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+import oracle
+import paper_1802_05065_b200 as fpt
+
+pytestmark = pytest.mark.gpu
+
+WANTED = [x for x in os.environ.get("FPT_FULLSIZE", "").split(",") if x]
+N_SAMPLE = {"c3": 48, "c5": 48, "c4": 16}
+OUT_DIR = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+
+
+def _oracle_ids(w, ids):
+    """The oracle on scattered ids, one trajectory per host thread (ctypes releases the GIL)."""
+    def one(i):
+        p = oracle.make_params(**dict(w["params"], first_id=int(i)))
+        r = oracle.simulate(p, 1, w["seed"], w["t_max"], nthreads=1)
+        return int(r["status"][0]), int(r["k"][0]), float(r["fpt"][0]), float(r["gamma"][0])
+    with ThreadPoolExecutor(max(1, min(len(ids), os.cpu_count() or 1))) as ex:
+        return list(ex.map(one, ids))
+
+
+@pytest.mark.parametrize("name", ["c3", "c5", "c4"])
+def test_full_config(name):
+    if name not in WANTED:
+        pytest.skip("set FPT_FULLSIZE=c3,c5,c4 to run the full-size configs")
+    fpt.lib()
+    fpt.set_launch(0, 0, 0)
+    w = fpt.workload(name)
+    n = w["n_traj"]
+    dt = w["params"]["dt"]
+    p = fpt.make_params(**w["params"])
+    out = fpt.binding._alloc_outputs(n)
+    counts = None
+    rng = np.random.default_rng(2024)
+    ids = np.sort(np.concatenate([[0, n - 1], rng.choice(np.arange(1, n - 1), N_SAMPLE[name] - 2, replace=False)]))
+
+    peak, clk = (fpt.fp32_peak if w["params"]["precision"] == "fp32" else fpt.fp64_peak)(1.0)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    if w.get("hist"):
+        of, lo, hi, nb = w["hist"]
+        counts = torch.zeros(nb + 2, dtype=torch.int64, device="cuda")
+        fpt.simulate_hist(p, n, w["seed"], w["t_max"], lo, hi, nb, hist_of=of, counts=counts, out=out)
+    else:
+        fpt.simulate(p, n, w["seed"], w["t_max"], out=out)
+    e1.record()
+    ora = _oracle_ids(w, ids)                      # host cores work while the kernel runs
+    t_oracle = time.perf_counter() - t0
+    e1.synchronize()
+    sec = e0.elapsed_time(e1) * 1e-3
+    st = fpt.last_stats()
+    f, g, s = (t.cpu().numpy() for t in out)
+
+    # ---- sampled ids against the oracle: bit-identical
+    bad = []
+    for i, (o_s, o_k, o_f, o_g) in zip(ids, ora):
+        if not (s[i] == o_s and f[i] == o_f and g[i] == o_g):
+            bad.append((int(i), int(s[i]), float(f[i]), float(g[i]), o_s, o_f, o_g))
+    assert not bad, bad
+
+    # ---- what holds at any size
+    esc = s == 0
+    k = np.where(esc, np.rint(f / dt), float(st["n_cap"])).astype(np.int64)
+    assert st["useful_steps"] == int(k.sum())
+    assert st["n_escaped"] == int(esc.sum()) and st["n_censored"] == int((s == 1).sum()) and st["n_nan"] == 0
+    assert np.all(f[s == 1] == -1.0) and np.all(f[esc] > 0) and np.all(k[esc] <= st["n_cap"])
+    rec_hist = None
+    if counts is not None:
+        c = counts.cpu().numpy().astype(np.uint64)
+        assert np.array_equal(c, oracle.histogram(g, s, lo, hi, nb))          # integer counts: exact
+        assert int(c.sum()) == int(esc.sum())
+        rec_hist = {"lo": lo, "hi": hi, "nbins": nb, "mean": float(g[esc].mean()), "std": float(g[esc].std()),
+                    "nonzero_bins": int((c[1:-1] > 0).sum()), "under": int(c[0]), "over": int(c[-1])}
+
+    steps_per_s = st["useful_steps"] / sec
+    rec = {"config": name, "n_traj": n, "seed": w["seed"], "t_max": w["t_max"], "seconds": sec, "steps": st["useful_steps"],
+           "steps_per_s": steps_per_s, "escapes_per_s": st["n_escaped"] / sec, "escaped": st["n_escaped"],
+           "censored": st["n_censored"], "lane_efficiency": st["lane_efficiency"], "migrations": st["migrations"],
+           "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"]},
+           "roofline_frac": steps_per_s * w["n64_ref"] / peak, "n_ref_per_step": w["n64_ref"], "peak_inst_per_s": peak,
+           "sm_clock_hz_seen": clk, "mean_steps": float(k.mean()), "min_steps": int(k.min()), "max_steps": int(k.max()),
+           "hist": rec_hist, "oracle_sampled_ids": len(ids), "oracle_seconds": t_oracle, "oracle_cores": os.cpu_count(),
+           "oracle_steps_per_s": float(sum(o[1] for o in ora)) / t_oracle}
+    os.makedirs(OUT_DIR, exist_ok=True)
+    with open(os.path.join(OUT_DIR, f"fullsize_{name}.json"), "w") as fh:
+        json.dump(rec, fh, indent=1)
+    print(json.dumps(rec))

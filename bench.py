@@ -219,7 +219,7 @@ def main():
         torch.cuda.synchronize()
 
     # ---- device-timed region: exactly K steps
-    first_id = rank * n_traj
+    first_id = fpt.sharding.shard_range(n_traj * world, rank, world)[0]      # rank r integrates ids [r*n, (r+1)*n)
     time_workload(fpt, torch, w, n_traj, 0, args.warmup, flush, first_id)          # warm-up
     sampler = ClockSampler(local_rank)
     barrier()

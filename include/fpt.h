@@ -122,6 +122,17 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
  * calculator), max_blocks (0 = no extra cap).  FPT_E_INVALID on a bad value. */
 int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks);
 
+/* Scheduler of subsequent fpt_simulate* calls of this process (results never depend on it; only the time does):
+ *   FPT_SCHEDULE_DYNAMIC (default) a finished lane takes the next id from a global counter at once, and
+ *                        sparse warps hand their trajectories over in the drain phase;
+ *   FPT_SCHEDULE_STATIC  the static split analysed in the paper's Appendix A: lane j of L owns runs
+ *                        j, j+L, j+2L, ...; nothing is handed over, a warp lives as long as its slowest lane.  With one
+ *                        run per lane this is the paper's own kernel (one thread per realisation).  It exists
+ *                        to measure what the dynamic scheduler buys (fpt_stats lane efficiency against Eq. (A.5)). */
+#define FPT_SCHEDULE_DYNAMIC 0
+#define FPT_SCHEDULE_STATIC  1
+int fpt_set_schedule(int32_t schedule);
+
 /* Synchronises the current device and returns the counters of the most recent fpt_simulate* call on it. */
 int fpt_last_stats(fpt_stats* out);
 

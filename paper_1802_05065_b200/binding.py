@@ -53,6 +53,7 @@ _SIGNATURES = {
     "fpt_simulate_host": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p],
     "fpt_set_launch": [C.c_int32, C.c_int32, C.c_int32],
+    "fpt_set_schedule": [C.c_int32],
     "fpt_last_stats": [C.POINTER(FptStats)],
     "fpt_fp64_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
     "fpt_fp32_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
@@ -169,6 +170,15 @@ def simulate_host(params: FptParams, n_traj: int, seed: int, t_max: float, fpt, 
 
 def set_launch(block=0, blocks_per_sm=0, max_blocks=0):
     _check(lib().fpt_set_launch(block, blocks_per_sm, max_blocks), "fpt_set_launch")
+
+
+SCHEDULE = {"dynamic": 0, "static": 1}
+
+
+def set_schedule(schedule="dynamic"):
+    """fpt_set_schedule: "dynamic" (refill + drain compaction, default) or "static" (Appendix A's split, for the A/B)."""
+    v = SCHEDULE[schedule] if isinstance(schedule, str) else int(schedule)
+    _check(lib().fpt_set_schedule(v), "fpt_set_schedule")
 
 
 def last_stats() -> dict:

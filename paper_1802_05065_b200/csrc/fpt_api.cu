@@ -32,6 +32,7 @@ constexpr int kDefaultK = 16;
 
 struct LaunchCfg {
   int block = 0, blocks_per_sm = 0, max_blocks = 0;
+  int schedule = 0;
 };
 std::mutex g_mu;
 LaunchCfg g_cfg;
@@ -232,6 +233,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     if (blocks > needed) blocks = needed;
     if (cfg.max_blocks > 0 && blocks > cfg.max_blocks) blocks = cfg.max_blocks;
     grid = (int)blocks;
+    P.schedule = cfg.schedule;
     void* args[] = {(void*)&P};
     FPT_CUDA(cudaLaunchKernel(fn, dim3(grid), dim3(block), args, smem, stream));
   }
@@ -549,6 +551,13 @@ int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks) {
   g_cfg.block = block;
   g_cfg.blocks_per_sm = blocks_per_sm;
   g_cfg.max_blocks = max_blocks;
+  return FPT_OK;
+}
+
+int fpt_set_schedule(int32_t schedule) {
+  if (schedule != FPT_SCHEDULE_DYNAMIC && schedule != FPT_SCHEDULE_STATIC) return FPT_E_INVALID;
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_cfg.schedule = schedule;
   return FPT_OK;
 }
 

@@ -13,6 +13,7 @@ namespace fpt {
 
 constexpr int kStatusEscaped = 0, kStatusCensored = 1, kStatusNan = 2;
 constexpr int kMaxFusedBins = 8192;
+constexpr int kScheduleDynamic = 0, kScheduleStatic = 1;
 
 struct DevStats {                 // device-side counters, one block of 8 x u64
   unsigned long long next_id;     // the global trajectory counter (S7)
@@ -27,6 +28,7 @@ struct KParams {
   unsigned long long n_traj, first_id, n_cap;
   int K;                          // poll interval in steps, a multiple of the macro step
   int hist_of;                    // -1 none, 0 gamma at escape, 1 escape time
+  int schedule;                   // kScheduleDynamic (refill from the global counter + drain compaction) | kScheduleStatic
   int nbins;
   double hist_lo, hist_scale;
   double* out_fpt;
@@ -267,6 +269,8 @@ __global__ void FPT_LAUNCH_BOUNDS fpt_persistent_kernel(const __grid_constant__ 
   bool active = false;                  // lane holds a live trajectory
   bool exhausted = false;               // warp-uniform: the global counter has run past n_traj
   unsigned long long idx = 0;           // index of the lane's trajectory within this call (id = first_id + idx)
+  const unsigned long long lanes_total = (unsigned long long)gridDim.x * blockDim.x;
+  unsigned long long next_static = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;   // static schedule only
   unsigned long long kbase = 0;         // steps completed by the lane's trajectory at the last poll
   uint32_t id_lo = 0, id_hi = 0;
   unsigned long long s_useful = 0, s_blocks = 0;
@@ -282,34 +286,44 @@ __global__ void FPT_LAUNCH_BOUNDS fpt_persistent_kernel(const __grid_constant__ 
     const unsigned want = __ballot_sync(0xffffffffu, !active);
     if (want) {
       if (!exhausted) {
-        const int leader = __ffs(want) - 1;
-        const unsigned cnt = __popc(want);
-        unsigned long long base = 0;
-        if ((int)lane == leader) {
-          base = atomicAdd(&P.ws->next_id, (unsigned long long)cnt);
-          ++s_atom;
-        }
-        base = __shfl_sync(0xffffffffu, base, leader);
-        if (!active) {
-          const unsigned long long mine = base + (unsigned long long)__popc(want & lt_mask);
-          if (mine < P.n_traj) {
-            idx = mine;
-            const unsigned long long id = P.first_id + mine;
-            id_lo = (uint32_t)id;
-            id_hi = (uint32_t)(id >> 32);
-            kbase = 0;
-            st.init(P);
-            active = true;
-            uint32_t o0, o1, o2, o3;                              // normals of block 0 of the new stream
-            philox_block(P.keys, 0u, 0u, id_lo, id_hi, o0, o1, o2, o3);
-            S::normals(o0, o1, o2, o3, zc);
+        unsigned long long mine = ~0ull;
+        if (P.schedule == kScheduleDynamic) {
+          const int leader = __ffs(want) - 1;
+          const unsigned cnt = __popc(want);
+          unsigned long long base = 0;
+          if ((int)lane == leader) {
+            base = atomicAdd(&P.ws->next_id, (unsigned long long)cnt);
+            ++s_atom;
           }
+          base = __shfl_sync(0xffffffffu, base, leader);
+          if (!active) mine = base + (unsigned long long)__popc(want & lt_mask);
+          exhausted = (base + cnt >= P.n_traj);
+        } else {
+          // static split of the paper's Appendix A: thread j owns runs j, j + L, j + 2L, ... (L lanes)
+          if (!active) {
+            mine = next_static;
+            next_static += lanes_total;
+          }
+          exhausted = __all_sync(0xffffffffu, next_static >= P.n_traj);
         }
-        exhausted = (base + cnt >= P.n_traj);
+        if (!active && mine < P.n_traj) {
+          idx = mine;
+          const unsigned long long id = P.first_id + mine;
+          id_lo = (uint32_t)id;
+          id_hi = (uint32_t)(id >> 32);
+          kbase = 0;
+          st.init(P);
+          active = true;
+          uint32_t o0, o1, o2, o3;                              // normals of block 0 of the new stream
+          philox_block(P.keys, 0u, 0u, id_lo, id_hi, o0, o1, o2, o3);
+          S::normals(o0, o1, o2, o3, zc);
+        }
       }
       // ---- drain: lanes that could not be refilled adopt parked trajectories; a sparse warp parks its own and retires
       const unsigned idle = __ballot_sync(0xffffffffu, !active);
-      if (idle) {                                           // implies exhausted
+      if (idle && P.schedule != kScheduleDynamic) {         // static split: no hand-over, the warp lives as long as its slowest lane
+        if (idle == 0xffffffffu && exhausted) break;
+      } else if (idle) {                                    // implies exhausted
         if (lane == 0)
           while (atomicCAS(&pool.lock, 0, 1) != 0) __nanosleep(64);
         __syncwarp();

@@ -6,7 +6,8 @@ the dynamic refill scheduler, on an imbalanced (near-exponential) workload.
     lengths (lane j of L owns runs j, j+L, ...; a warp lasts as long as its slowest lane; poll granularity K);
   * its lane efficiency follows the closed form of Appendix A, oracle/appendix_a.py, for N_tpb = 32 (a warp), within
     the few per cent by which the escape-time law differs from an exponential (PAPER.md:417 says so itself);
-  * the dynamic scheduler stays above 90 % on the same work.
+  * the dynamic scheduler (refill + drain compaction) stays above 85 % / 95 % with 4 / 16 runs per lane, where the static
+    split sits near 43 % / 63 %.
 """
 import numpy as np
 import pytest
@@ -49,7 +50,7 @@ def _static_issued(k_end, lanes, K):
 def test_static_split_matches_appendix_a_and_dynamic_beats_it(runs_per_lane):
     # overdamped washboard, gamma = 0.7, T = 0.08: mean ~1e5 steps, escape times exponential to a few per cent; no cap in reach
     w = fpt.workload("c5", temperature=0.08, t_max=5e-3 * 4e7)
-    blocks, block = 64, 64
+    blocks, block = 16, 256                                        # 8 warps per block: drain compaction has room
     lanes = blocks * block
     n = lanes * runs_per_lane
     fs, gs, ss, st_static = _run(w, n, "static", (block, 0, blocks))
@@ -73,4 +74,4 @@ def test_static_split_matches_appendix_a_and_dynamic_beats_it(runs_per_lane):
     # what the refill scheduler buys on the same trajectories
     assert st_dyn["lane_efficiency"] > st_static["lane_efficiency"]
     if runs_per_lane >= 4:
-        assert st_dyn["lane_efficiency"] > 0.9, st_dyn
+        assert st_dyn["lane_efficiency"] > (0.85 if runs_per_lane == 4 else 0.95), st_dyn

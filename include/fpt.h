@@ -117,6 +117,20 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
                       double* h_fpt, double* h_gamma_at_escape, int32_t* h_status,
                       int32_t hist_of, double lo, double hi, int32_t nbins, uint64_t* h_counts);
 
+/* Parameter-sweep batch: n_sets independent jobs of n_per_set trajectories each, e.g. the temperature sweep behind the
+ * Arrhenius / Kramers plot of the mean escape time (Eqs. (12)-(14), Fig. 10) or a sweep of the bias.
+ * Set s uses sets[s] (any field may differ between sets, including model and scheme), the cap t_max[s] and the ids
+ * sets[s].first_id + 0 .. n_per_set-1 of the Philox stream `seed`: give the sets disjoint id ranges for independent
+ * samples, equal ranges for common random numbers.  Outputs of set s occupy elements [s*n_per_set, (s+1)*n_per_set) of
+ * the out_* arrays (device, n_sets*n_per_set elements; out_gamma_at_escape may be NULL).  The sets run CONCURRENTLY as
+ * separate persistent launches on an internal pool of streams (a small set cannot fill 148 SMs, and each launch lasts as
+ * long as its longest trajectory), forked from and joined back into cuda_stream, so to the caller this is one
+ * asynchronous call like fpt_simulate.  Each result is bit-identical to a separate fpt_simulate of that set.
+ * sets and t_max are host arrays read during the call.  FPT_E_INVALID as fpt_simulate for any set (nothing is
+ * launched then), or NULL sets / t_max, n_sets < 0.  fpt_last_stats afterwards describes one of the sets. */
+int fpt_simulate_sweep(const fpt_params* sets, int32_t n_sets, int64_t n_per_set, uint64_t seed, const double* t_max,
+                       double* out_fpt, double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream);
+
 /* Launch geometry override for subsequent fpt_simulate* calls of this process (results never depend on it):
  * block = threads per block (multiple of 32, 32..256; 0 = default), blocks_per_sm (0 = default from the occupancy
  * calculator), max_blocks (0 = no extra cap).  FPT_E_INVALID on a bad value. */

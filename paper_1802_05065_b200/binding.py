@@ -52,6 +52,8 @@ _SIGNATURES = {
     "fpt_histogram": [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_simulate_host": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p],
+    "fpt_simulate_sweep": [C.POINTER(FptParams), C.c_int32, C.c_int64, C.c_uint64, C.POINTER(C.c_double), C.c_void_p,
+                           C.c_void_p, C.c_void_p, C.c_void_p],
     "fpt_set_launch": [C.c_int32, C.c_int32, C.c_int32],
     "fpt_set_schedule": [C.c_int32],
     "fpt_last_stats": [C.POINTER(FptStats)],
@@ -166,6 +168,22 @@ def simulate_host(params: FptParams, n_traj: int, seed: int, t_max: float, fpt, 
         h = HIST_OF[h] if isinstance(h, str) else int(h)
     _check(lib().fpt_simulate_host(C.byref(params), n_traj, seed, t_max, hp(fpt), hp(gamma), hp(status), h, lo, hi, nb,
                                    hp(cnt)), "fpt_simulate_host")
+
+
+def simulate_sweep(param_sets, n_per_set: int, seed: int, t_max, out=None, stream=None):
+    """fpt_simulate_sweep.  param_sets: sequence of FptParams; t_max: one cap or one per set.  Returns (fpt, gamma,
+    status) CUDA tensors of shape (n_sets, n_per_set).  Asynchronous."""
+    n_sets = len(param_sets)
+    arr = (FptParams * max(1, n_sets))(*param_sets)
+    caps = [float(t_max)] * n_sets if not hasattr(t_max, "__len__") else [float(x) for x in t_max]
+    if len(caps) != n_sets:
+        raise ValueError("t_max must be a scalar or have one entry per parameter set")
+    tm = (C.c_double * max(1, n_sets))(*caps)
+    fpt, gam, st = out if out is not None else _alloc_outputs(n_sets * n_per_set)
+    _check(lib().fpt_simulate_sweep(arr, n_sets, n_per_set, seed, tm, _ptr(fpt), _ptr(gam), _ptr(st), _stream(stream)),
+           "fpt_simulate_sweep")
+    shape = (n_sets, n_per_set)
+    return fpt.view(shape), (gam.view(shape) if gam is not None else None), st.view(shape)
 
 
 def set_launch(block=0, blocks_per_sm=0, max_blocks=0):

@@ -37,7 +37,13 @@ struct LaunchCfg {
 std::mutex g_mu;
 LaunchCfg g_cfg;
 
-struct DeviceCtx {          // per device: the "last call" counters
+constexpr int kSweepStreams = 8;
+
+struct DeviceCtx {          // per device: the "last call" counters, and the stream pool of fpt_simulate_sweep
+  cudaStream_t pool[kSweepStreams] = {};
+  cudaEvent_t pool_done[kSweepStreams] = {};
+  cudaEvent_t fork = nullptr;
+  bool pool_ready = false;
   DevStats* d_last = nullptr;
   fpt_stats host{};         // geometry etc. filled at launch, counters read back on demand
   cudaStream_t last_stream = nullptr;
@@ -541,6 +547,47 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
   e = cudaStreamSynchronize(stream);
   cudaStreamDestroy(stream);
   if (rc == FPT_OK && e != cudaSuccess) { g_last_cuda = e; (void)cudaGetLastError(); return FPT_E_CUDA; }
+  return rc;
+}
+
+int fpt_simulate_sweep(const fpt_params* sets, int32_t n_sets, int64_t n_per_set, uint64_t seed, const double* t_max,
+                       double* out_fpt, double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream) {
+  if (!sets || !t_max || n_sets < 0 || n_per_set < 0) return FPT_E_INVALID;
+  for (int32_t i = 0; i < n_sets; ++i) {                       // nothing is launched unless every set is valid
+    const int rc = validate(&sets[i], n_per_set, t_max[i]);
+    if (rc != FPT_OK) return rc;
+  }
+  if (n_sets == 0 || n_per_set == 0) return FPT_OK;
+  if (!out_fpt || !out_status) return FPT_E_INVALID;
+  DeviceCtx* ctx = nullptr;
+  int rc = device_ctx(&ctx);
+  if (rc != FPT_OK) return rc;
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (!ctx->pool_ready) {
+      for (int i = 0; i < kSweepStreams; ++i) {
+        FPT_CUDA(cudaStreamCreateWithFlags(&ctx->pool[i], cudaStreamNonBlocking));
+        FPT_CUDA(cudaEventCreateWithFlags(&ctx->pool_done[i], cudaEventDisableTiming));
+      }
+      FPT_CUDA(cudaEventCreateWithFlags(&ctx->fork, cudaEventDisableTiming));
+      ctx->pool_ready = true;
+    }
+  }
+  cudaStream_t caller = (cudaStream_t)cuda_stream;
+  const int used = n_sets < kSweepStreams ? n_sets : kSweepStreams;
+  // fork: the pool streams start after everything already queued on the caller's stream
+  FPT_CUDA(cudaEventRecord(ctx->fork, caller));
+  for (int i = 0; i < used; ++i) FPT_CUDA(cudaStreamWaitEvent(ctx->pool[i], ctx->fork, 0));
+  for (int32_t i = 0; i < n_sets && rc == FPT_OK; ++i) {
+    const size_t off = (size_t)i * (size_t)n_per_set;
+    rc = simulate_impl(&sets[i], n_per_set, seed, t_max[i], out_fpt + off, out_gamma_at_escape ? out_gamma_at_escape + off : nullptr,
+                       out_status + off, false, 0, 0.0, 0.0, 0, nullptr, ctx->pool[i % kSweepStreams]);
+  }
+  // join: the caller's stream continues when every set is done (also after a failed launch, so nothing dangles)
+  for (int i = 0; i < used; ++i) {
+    FPT_CUDA(cudaEventRecord(ctx->pool_done[i], ctx->pool[i]));
+    FPT_CUDA(cudaStreamWaitEvent(caller, ctx->pool_done[i], 0));
+  }
   return rc;
 }
 

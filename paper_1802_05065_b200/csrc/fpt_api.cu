@@ -216,8 +216,10 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
       // one runs fastest when few warps share its SM sub-partition; the refills keep the lanes busy meanwhile).
       const long long R = ramp ? 1 : 5;
       const long long unit = 128LL * sms;                       // one warp per sub-partition everywhere
-      long long units = n_traj / (R * unit);
-      if (units >= 1) {
+      // ramped: round UP, so that a job that fits resident at once runs as one wave (C4: 65536 equal-length trajectories
+      // on 4 x 128 lanes per SM, not 3 x 128 plus a straggler wave); constant bias: round down, more refills per lane
+      long long units = ramp ? (n_traj + unit - 1) / unit : n_traj / (R * unit);
+      if (n_traj >= unit && units >= 1) {
         int per_sm128 = 0;
         FPT_CUDA(max_blocks_per_sm(128, &per_sm128));
         if (per_sm128 < 1) return FPT_E_CUDA;

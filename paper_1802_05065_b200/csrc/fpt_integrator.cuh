@@ -222,6 +222,10 @@ __device__ __forceinline__ int hist_slot(double x, double lo, double scale, int 
 #ifndef FPT_LB_MINBLOCKS
 #define FPT_LB_MINBLOCKS 1
 #endif
+#ifndef FPT_UNROLL
+#define FPT_UNROLL 4
+#endif
+constexpr int kUnroll = FPT_UNROLL;     // macro steps per trip of the step loop (a larger basic block schedules better)
 constexpr int kMaxWarpsPerBlock = FPT_LB_THREADS / 32;
 
 // Drain-phase lane compaction (per block, shared memory).  Once the global id counter is exhausted a warp cannot refill
@@ -393,7 +397,7 @@ __global__ void FPT_LAUNCH_BOUNDS fpt_persistent_kernel(const __grid_constant__ 
     int koff = 0;                       // step offset (1..K) of the first capture in this interval, 0 = none
     int cap_hi = 0;                     // high word of phi at the capture (distinguishes a crossing from a NaN)
     bool captured = false;
-#pragma unroll 1
+#pragma unroll(kUnroll)
     for (int jj = 0; jj < n_macro; ++jj) {
       const unsigned long long bn = b0 + (unsigned long long)(jj + 1);
       uint32_t o0, o1, o2, o3;

@@ -56,10 +56,10 @@ __global__ void __launch_bounds__(256) mix_kernel(double* sink, int iters, doubl
 }
 
 template <int MODE>
-void run(const char* name, double sm_clock_hz) {
+void run(const char* name, double sm_clock_hz, int block = 256, int per_sm = 4) {
   double* sink = nullptr;
   cudaMalloc(&sink, 8);
-  const int iters = 2000, block = 256, per_sm = 4;
+  const int iters = 2000;
   int sms = 0;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
   cudaEvent_t e0, e1;
@@ -78,7 +78,7 @@ void run(const char* name, double sm_clock_hz) {
     if (ms < best) best = ms;
   }
   const double groups_per_warp = (double)iters * 32, warps_per_subpartition = (double)per_sm * block / 32 / 4;
-  printf("| %-28s | %8.3f | %6.2f |\n", name, best, best * 1e-3 * sm_clock_hz / (groups_per_warp * warps_per_subpartition));
+  printf("| %-28s (%2d warps/sub-partition) | %8.3f | %6.2f |\n", name, per_sm * block / 128, best, best * 1e-3 * sm_clock_hz / (groups_per_warp * warps_per_subpartition));
   cudaFree(sink);
 }
 
@@ -105,5 +105,15 @@ int main(int argc, char** argv) {
   run<D | W | L>("DFMA + IMAD.WIDE + LOP3", clk);
   run<D | D2 | L>("2 DFMA + LOP3", clk);
   run<D | D3 | L>("3 DFMA + LOP3", clk);
+  // how many warps the FP64 pipe needs: DFMA only (8 independent chains per thread) at 1 .. 16 warps per sub-partition
+  run<D>("DFMA", clk, 128, 1);
+  run<D>("DFMA", clk, 128, 2);
+  run<D>("DFMA", clk, 128, 3);
+  run<D>("DFMA", clk, 128, 4);
+  run<D>("DFMA", clk, 256, 4);
+  run<D>("DFMA", clk, 256, 8);
+  run<D | L>("DFMA + LOP3", clk, 128, 1);
+  run<D | L>("DFMA + LOP3", clk, 128, 4);
+  run<D | L>("DFMA + LOP3", clk, 256, 8);
   return 0;
 }

@@ -111,12 +111,25 @@ def oracle_rate(w: dict, budget_s: float, n_max: int, first_id: int = 0):
     return steps / dt0, float(np.sum(r["status"] == 0)) / dt0, n, dt0, cores
 
 
+TWINS = {"c3_fast": ("c3", dict(nu=1e-3, t_max=1050.0), 1 << 19),
+         "c5_T0.1": ("c5", dict(temperature=0.1, t_max=2000.0), 1 << 20),
+         "c4_fast": ("c4", dict(nu=1e-4, t_max=5500.0), 1 << 18)}
+
+
+def resolve_workload(fpt, name: str):
+    """(workload dict, trajectory count of a throughput-shaped twin or None)."""
+    if name in TWINS:
+        base, ov, n = TWINS[name]
+        return fpt.workload(base, **ov), n
+    return fpt.workload(name), None
+
+
 def run_reference(args, rank: int):
     """--impl reference: the oracle on the host cores (rank 0 only)."""
     if rank != 0:
         return
     import paper_1802_05065_b200 as fpt
-    w = fpt.workload(args.workload)
+    w, _ = resolve_workload(fpt, args.workload)
     per_step_budget = max(1.0, min(15.0, 90.0 / max(1, args.steps + args.warmup)))
     rates, esc, ids, secs = [], [], 0, 0.0
     cores = host_cores()
@@ -174,7 +187,10 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5", "c3_fast", "c4_fast", "c5_T0.1"],
+                    help="c2 = BASELINE.json configs[1] (the metric's workload).  c3/c4/c5 are the FULL configs' parameters on 65536 "
+                         "ids (minutes to hours per step); the *_fast / c5_T0.1 twins keep every parameter but the ramp rate / "
+                         "temperature, so a step lasts ~0.1-0.3 s (what the extra_workloads block and the ncu captures use)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-traj", type=int, default=0, help="override the trajectories per step (0 = the config's own count)")
     ap.add_argument("--no-extra", action="store_true", help="skip the throughput-shaped extra workloads and the CPU baseline")
@@ -201,8 +217,8 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    w = fpt.workload(args.workload)
-    n_traj = w["n_traj"]
+    w, n_twin = resolve_workload(fpt, args.workload)
+    n_traj = n_twin or w["n_traj"]
     if args.workload in ("c3", "c4", "c5"):       # full configs take minutes: bench them on a fixed id range
         n_traj = min(n_traj, 1 << 16)
     if args.n_traj > 0:
@@ -266,7 +282,8 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: BASELINE.json configs[{int(args.workload[1]) - 1}]", "n_traj_per_gpu": n_traj,
+        "config": {"workload": f"{args.workload}: BASELINE.json configs[{int(args.workload[1]) - 1}]"
+                               + (" parameters, scaled twin" if args.workload in TWINS else ""), "n_traj_per_gpu": n_traj,
                    "seed": w["seed"], "t_max": w["t_max"], "params": {k2: v for k2, v in w["params"].items()},
                    "l2": "no input arrays (inputs are generated in-kernel from seed and id); 256 MiB written between timed steps",
                    "parallelism": f"independent id ranges x{world}, no collective"},
@@ -296,9 +313,9 @@ def main():
         # ---- throughput-shaped workloads (same parameters as the configs, id ranges sized to fill the GPU for ~0.1-1 s)
         extra = {}
         shapes = [("c2_x42", "c2", dict(), 1 << 22, False),
-                  ("c3_fast_ramp", "c3", dict(nu=1e-3, t_max=1050.0), 1 << 19, True),
-                  ("c5_T0.1", "c5", dict(temperature=0.1, t_max=2000.0), 1 << 20, False),
-                  ("c4_fast_ramp", "c4", dict(nu=1e-4, t_max=5500.0), 1 << 18, False)]
+                  ("c3_fast_ramp",) + TWINS["c3_fast"] + (True,),
+                  ("c5_T0.1",) + TWINS["c5_T0.1"] + (False,),
+                  ("c4_fast_ramp",) + TWINS["c4_fast"] + (False,)]
         for name, base, ov, n, hist in shapes:
             ww = fpt.workload(base, **ov)
             r = time_workload(fpt, torch, ww, n, 3, 1, flush, 0, hist=hist)

@@ -115,5 +115,13 @@ int main(int argc, char** argv) {
   run<D | L>("DFMA + LOP3", clk, 128, 1);
   run<D | L>("DFMA + LOP3", clk, 128, 4);
   run<D | L>("DFMA + LOP3", clk, 256, 8);
+  // fp32 variant: FFMA next to the integer classes
+  run<F | L>("FFMA + LOP3", clk);
+  run<F2 | L>("2 FFMA + LOP3", clk);
+  run<F3 | L>("3 FFMA + LOP3", clk);
+  run<F | W>("FFMA + IMAD.WIDE", clk);
+  run<F3 | W>("3 FFMA + IMAD.WIDE", clk);
+  run<F3 | F2 | F | W | L>("6 FFMA + IMAD.WIDE + LOP3", clk);
+  run<F3 | F2 | F | L | L2>("6 FFMA + 2 LOP3", clk);
   return 0;
 }

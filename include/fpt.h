@@ -83,6 +83,8 @@ typedef struct fpt_stats {
   int32_t  check_every;        /* effective K                                                             */
   int32_t  reserved;
   uint64_t migrations;         /* trajectories parked by a sparse warp and adopted by another (drain-phase compaction) */
+  uint64_t helper_lane_steps;  /* 32 * (steps whose normals a tail-helper warp generated for its block's last live warp);
+                                  NOT part of issued_lane_steps                                            */
 } fpt_stats;
 
 /* Integrate trajectories id = first_id .. first_id+n_traj-1 until first passage or the cap n_cap = nearbyint(t_max/dt).
@@ -146,6 +148,12 @@ int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks);
 #define FPT_SCHEDULE_DYNAMIC 0
 #define FPT_SCHEDULE_STATIC  1
 int fpt_set_schedule(int32_t schedule);
+
+/* Tail helper (default on; results never depend on it): when a block is down to one live warp and nothing is parked, a
+ * retired warp of the block generates that warp's normals (Philox + Box-Muller) one chunk ahead into shared memory and the
+ * survivor only integrates, which shortens the time a launch waits for its longest trajectories.  Needs blocks of at least
+ * two warps and a poll interval that is a multiple of 32 steps; otherwise it stays off by itself. */
+int fpt_set_tail_helper(int32_t on);
 
 /* Synchronises the current device and returns the counters of the most recent fpt_simulate* call on it. */
 int fpt_last_stats(fpt_stats* out);

@@ -6,6 +6,6 @@ fallback: importing works without the library, but the first call raises if it h
 """
 from .binding import (FptError, FptParams, FptStats, dbg_normals_f32, dbg_normals_f64, dbg_philox, dbg_selfcheck, dbg_sincos_f32,  # noqa: F401
                       dbg_sincos_f64, dbg_trace, dbg_unary_f32, dbg_unary_f64, fp32_peak, fp64_peak, histogram, last_stats,
-                      lib, make_params, set_launch, set_schedule, simulate, simulate_hist, simulate_host, simulate_sweep, version)
+                      lib, make_params, set_launch, set_schedule, set_tail_helper, simulate, simulate_hist, simulate_host, simulate_sweep, version)
 from . import analysis, sharding, units  # noqa: F401
 from .workloads import CONFIGS, workload  # noqa: F401

@@ -35,7 +35,7 @@ class FptStats(C.Structure):
     _fields_ = [("n_traj", C.c_uint64), ("n_escaped", C.c_uint64), ("n_censored", C.c_uint64), ("n_nan", C.c_uint64),
                 ("useful_steps", C.c_uint64), ("issued_lane_steps", C.c_uint64), ("refill_atomics", C.c_uint64),
                 ("n_cap", C.c_uint64), ("grid", C.c_int32), ("block", C.c_int32), ("check_every", C.c_int32),
-                ("reserved", C.c_int32), ("migrations", C.c_uint64)]
+                ("reserved", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64)]
 
     def as_dict(self):
         d = {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
@@ -56,6 +56,7 @@ _SIGNATURES = {
                            C.c_void_p, C.c_void_p, C.c_void_p],
     "fpt_set_launch": [C.c_int32, C.c_int32, C.c_int32],
     "fpt_set_schedule": [C.c_int32],
+    "fpt_set_tail_helper": [C.c_int32],
     "fpt_last_stats": [C.POINTER(FptStats)],
     "fpt_fp64_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
     "fpt_fp32_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
@@ -197,6 +198,10 @@ def set_schedule(schedule="dynamic"):
     """fpt_set_schedule: "dynamic" (refill + drain compaction, default) or "static" (Appendix A's split, for the A/B)."""
     v = SCHEDULE[schedule] if isinstance(schedule, str) else int(schedule)
     _check(lib().fpt_set_schedule(v), "fpt_set_schedule")
+
+
+def set_tail_helper(on=True):
+    _check(lib().fpt_set_tail_helper(1 if on else 0), "fpt_set_tail_helper")
 
 
 def last_stats() -> dict:

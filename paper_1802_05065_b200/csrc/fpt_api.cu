@@ -35,6 +35,7 @@ constexpr int kDefaultK64 = 64, kDefaultK32 = 32;
 struct LaunchCfg {
   int block = 0, blocks_per_sm = 0, max_blocks = 0;
   int schedule = 0;
+  int tail_helper = 1;
 };
 std::mutex g_mu;
 LaunchCfg g_cfg;
@@ -244,6 +245,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     if (cfg.max_blocks > 0 && blocks > cfg.max_blocks) blocks = cfg.max_blocks;
     grid = (int)blocks;
     P.schedule = cfg.schedule;
+    P.tail_helper = cfg.tail_helper;
     void* args[] = {(void*)&P};
     FPT_CUDA(cudaLaunchKernel(fn, dim3(grid), dim3(block), args, smem, stream));
   }
@@ -612,6 +614,13 @@ int fpt_set_schedule(int32_t schedule) {
   return FPT_OK;
 }
 
+int fpt_set_tail_helper(int32_t on) {
+  if (on != 0 && on != 1) return FPT_E_INVALID;
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_cfg.tail_helper = on;
+  return FPT_OK;
+}
+
 int fpt_last_stats(fpt_stats* out) {
   if (!out) return FPT_E_INVALID;
   DeviceCtx* ctx = nullptr;
@@ -630,6 +639,7 @@ int fpt_last_stats(fpt_stats* out) {
   out->issued_lane_steps = h.issued_lane_steps;
   out->refill_atomics = h.refill_atomics;
   out->migrations = h.migrations;
+  out->helper_lane_steps = h.helper_lane_steps;
   return FPT_OK;
 }
 
@@ -645,7 +655,7 @@ const char* fpt_strerror(int code) {
   }
 }
 
-int fpt_version(void) { return 101; }
+int fpt_version(void) { return 102; }
 
 // ---- test hooks
 int fpt_dbg_philox(uint64_t seed, uint64_t id0, int64_t n_ids, uint64_t block, uint32_t* out, void* s) {

@@ -330,6 +330,45 @@ def test_drain_compaction_parks_and_adopts_without_changing_results():
             assert st["lane_efficiency"] > 0.5, st
 
 
+def test_tail_helper_serves_the_last_warp_without_changing_results():
+    """Tail helper: when a block is down to one live warp, its retired warps generate that warp's normals into shared
+    memory and the survivor only integrates.  Same stream positions, same arithmetic: results must stay the oracle's, with
+    the helper on and off, for fp64 and fp32 states, with and without a ramp; and the helper must actually engage."""
+    cases = [
+        (fpt.workload("c2", t_max=400.0), 1536, REL_FP64, 64),                               # fp64 Heun underdamped
+        (fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3), 768, REL_FP64, 128),                # fp64 ramp (gamma_k from k)
+        (fpt.workload("c5", temperature=0.1, t_max=1500.0), 1536, REL_FP64, 64),             # fp64 EM overdamped
+        (fpt.workload("c4", nu=2e-5, t_max=0.55 / 2e-5), 768, REL_FP32, 32),                 # fp32 + Kahan time, chunk of 32
+    ]
+    for w, n, rel, K in cases:
+        ora = run_oracle(w, n)
+        outs = []
+        for on in (True, False):
+            fpt.set_tail_helper(on)
+            fpt.set_launch(128, 1, n // 128)            # every trajectory resident: blocks of 4 warps drain down to one
+            try:
+                gpu = run_gpu(w, n, check_every=K)
+                st = fpt.last_stats()
+            finally:
+                fpt.set_launch(0, 0, 0)
+                fpt.set_tail_helper(True)
+            assert_parity(gpu, ora, w["params"]["dt"], rel)
+            assert st["useful_steps"] == int(np.sum(ora["k"]))
+            assert (st["helper_lane_steps"] > 0) == on, (on, st)
+            outs.append(gpu)
+        assert all(np.array_equal(a, b) for a, b in zip(*outs))
+    # a poll interval that is not a multiple of the hand-over chunk, or blocks of fewer than three warps: the helper stays off
+    w = fpt.workload("c2", t_max=100.0)
+    run_gpu(w, 512, check_every=48)
+    assert fpt.last_stats()["helper_lane_steps"] == 0
+    fpt.set_launch(64, 1, 8)
+    try:
+        run_gpu(w, 512, check_every=64)
+        assert fpt.last_stats()["helper_lane_steps"] == 0
+    finally:
+        fpt.set_launch(0, 0, 0)
+
+
 # edge and degenerate cases
 def test_edge_cases():
     w = fpt.workload("c2")

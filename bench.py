@@ -290,7 +290,7 @@ def main():
         "escapes_per_s": escaped_all * args.steps / dev_s,
         "censored": int(st["n_censored"]), "lane_efficiency": st["lane_efficiency"],
         "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"]},
-        "wall_s_timed_region": t_wall,
+        "wall_s_timed_region": t_wall, "ms_each_step": [round(x, 3) for x in res["ms"]],
         "e2e": {"value": useful_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 96,
                 "d2h_bytes_per_step": n_traj * 20, "api": "fpt_simulate_host (pinned host outputs; inputs = 96-byte fpt_params)"},
         "gpu_launches": args.steps,             # one persistent-kernel launch per step (plus a memset and a 64-byte D2D copy)

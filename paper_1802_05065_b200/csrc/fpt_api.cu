@@ -47,6 +47,7 @@ struct DeviceCtx {          // per device: the "last call" counters, and the str
   cudaEvent_t pool_done[kSweepStreams] = {};
   cudaEvent_t fork = nullptr;
   bool pool_ready = false;
+  cudaMemPool_t mem = nullptr;   // the library's own stream-ordered pool: freed blocks stay cached across synchronisations
   DevStats* d_last = nullptr;
   fpt_stats host{};         // geometry etc. filled at launch, counters read back on demand
   cudaStream_t last_stream = nullptr;
@@ -64,6 +65,17 @@ int device_ctx(DeviceCtx** out) {
     FPT_CUDA(cudaMalloc(&c.d_last, sizeof(DevStats)));
     FPT_CUDA(cudaMemset(c.d_last, 0, sizeof(DevStats)));
     FPT_CUDA(cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev));
+    // per-call workspaces come from a private memory pool that never trims (release threshold = max): with the device's
+    // default pool every stream synchronisation hands the memory back to the driver and the next call pays a real
+    // allocation (hundreds of microseconds, sometimes milliseconds) between the caller's event and the kernel launch
+    cudaMemPoolProps props{};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    FPT_CUDA(cudaMemPoolCreate(&c.mem, &props));
+    unsigned long long keep = ~0ull;
+    FPT_CUDA(cudaMemPoolSetAttribute(c.mem, cudaMemPoolAttrReleaseThreshold, &keep));
   }
   *out = &c;
   return FPT_OK;
@@ -173,7 +185,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     P.out_counts = (unsigned long long*)out_counts;
   }
   DevStats* ws = nullptr;
-  FPT_CUDA(cudaMallocAsync(&ws, sizeof(DevStats), stream));
+  FPT_CUDA(cudaMallocFromPoolAsync(&ws, sizeof(DevStats), ctx->mem, stream));
   FPT_CUDA(cudaMemsetAsync(ws, 0, sizeof(DevStats), stream));
   P.ws = ws;
 
@@ -525,12 +537,15 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
   if (rc != FPT_OK) return rc;
   if (n_traj == 0) return FPT_OK;
   if (!h_fpt || !h_status) return FPT_E_INVALID;
+  DeviceCtx* hctx = nullptr;
+  rc = device_ctx(&hctx);
+  if (rc != FPT_OK) return rc;
   cudaStream_t stream = nullptr;
   FPT_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
   const size_t n = (size_t)n_traj;
   const size_t bytes = n * (8 + (h_gamma ? 8 : 0) + 4) + (h_counts ? (size_t)(nbins > 0 ? nbins + 2 : 0) * 8 : 0);
   char* d = nullptr;
-  cudaError_t e = cudaMallocAsync(&d, bytes, stream);
+  cudaError_t e = cudaMallocFromPoolAsync((void**)&d, bytes, hctx->mem, stream);
   if (e != cudaSuccess) { g_last_cuda = e; cudaStreamDestroy(stream); return FPT_E_CUDA; }
   double* d_fpt = (double*)d;
   double* d_gam = h_gamma ? d_fpt + n : nullptr;

@@ -32,9 +32,9 @@ METRIC = "trajectory-steps/s"
 UNIT = "steps/s"
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE persistent-kernel launch of the bench workload (C2, 10^5 trajectories),
-# from the `ncu --set full` capture summarised in profiles/r01d_README.md: 39 680 B read, 0 B written (the 2 MB of outputs
+# from the `ncu --set full` capture summarised in profiles/r01e_README.md: 53 248 B read, 0 B written (the 2 MB of outputs
 # are still in the 126 MB L2 when the kernel ends).  Only valid for that workload; None for any other.
-NCU_DRAM_BYTES_PER_LAUNCH = 39680
+NCU_DRAM_BYTES_PER_LAUNCH = 53248
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -306,7 +306,7 @@ def main():
                 f"{'FFMA' if fp32 else 'DFMA'} chains measured live by fpt_fp{'32' if fp32 else '64'}_peak after 1 s of load "
                 f"(SM clock seen {clk_hz / 1e6:.0f} MHz); MEASURED_PEAKS.json has no {'FP32' if fp32 else 'FP64'} figure",
         "hbm_bytes_per_step_algorithmic": n_traj * 20,
-        "fp64_instr_per_step_in_sass": {"c1": 31.9, "c2": 73.9, "c3": 75.9, "c5": 48.9}.get(args.workload),
+        "fp64_instr_per_step_in_sass": {"c1": 31.4, "c2": 73.4, "c3": 75.4, "c5": 48.4}.get(args.workload),
     }
 
     if rank == 0 and world == 1 and not args.no_extra:

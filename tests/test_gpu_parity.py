@@ -369,6 +369,38 @@ def test_tail_helper_serves_the_last_warp_without_changing_results():
         fpt.set_launch(0, 0, 0)
 
 
+def test_concurrent_streams_and_host_threads():
+    """The calls are asynchronous on the caller's stream and the library keeps no per-call state outside its stream-ordered
+    workspace: launches queued on several streams, from several host threads, must give the results of the same calls
+    made one after the other."""
+    import threading
+    jobs = [(fpt.workload("c2", t_max=80.0), 3001, 11), (fpt.workload("c5", temperature=0.15, t_max=600.0), 2000, 12),
+            (fpt.workload("c3", nu=4e-3, t_max=1.05 / 4e-3), 1500, 13), (fpt.workload("c4", nu=5e-5, t_max=0.55 / 5e-5), 900, 14),
+            (fpt.workload("c1"), 4000, 15), (fpt.workload("c2", t_max=30.0, scheme="em"), 2500, 16)]
+    ref = []
+    for w, n, seed in jobs:
+        f, g, s = fpt.simulate(fpt.make_params(**w["params"]), n, seed, w["t_max"])
+        torch.cuda.synchronize()
+        ref.append((f.clone(), g.clone(), s.clone()))
+    streams = [torch.cuda.Stream() for _ in jobs]
+    outs = [None] * len(jobs)
+
+    def work(i):
+        w, n, seed = jobs[i]
+        with torch.cuda.stream(streams[i]):
+            for _ in range(3):                                   # back to back on the same stream as well
+                outs[i] = fpt.simulate(fpt.make_params(**w["params"]), n, seed, w["t_max"], stream=streams[i])
+
+    threads = [threading.Thread(target=work, args=(i,)) for i in range(len(jobs))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    torch.cuda.synchronize()
+    for (f, g, s), (rf, rg, rs) in zip(outs, ref):
+        assert torch.equal(s, rs) and torch.equal(f, rf) and torch.equal(g.nan_to_num(nan=-7.0), rg.nan_to_num(nan=-7.0))
+
+
 # edge and degenerate cases
 def test_edge_cases():
     w = fpt.workload("c2")

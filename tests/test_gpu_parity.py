@@ -401,6 +401,31 @@ def test_concurrent_streams_and_host_threads():
         assert torch.equal(s, rs) and torch.equal(f, rf) and torch.equal(g.nan_to_num(nan=-7.0), rg.nan_to_num(nan=-7.0))
 
 
+def test_random_geometries_poll_intervals_and_helper_settings_agree():
+    """Stress of the scheduling machinery (refill, parking / adoption, tail helper, lobby): 40 random launch geometries,
+    poll intervals and helper settings on workloads with escaped AND censored trajectories must all give the outputs of
+    the first run, bit for bit -- the outputs are a function of (params, seed, id) only."""
+    rng = np.random.default_rng(99)
+    for w, n in [(fpt.workload("c2", t_max=90.0), 5000), (fpt.workload("c5", temperature=0.12, t_max=250.0), 4000),
+                 (fpt.workload("c4", nu=2e-4, t_max=2220.0), 3000)]:
+        ref = run_gpu(w, n)
+        assert 0 < np.sum(ref[2] == 1) < n and np.sum(ref[2] == 0) > 0
+        for trial in range(40):
+            block = int(rng.choice([32, 64, 96, 128, 160, 192, 224, 256]))
+            per_sm = int(rng.choice([0, 1, 2, 3]))
+            max_blocks = int(rng.choice([0, 1, 3, 7, 20, 148]))
+            K = int(rng.choice([0, 4, 32, 64, 96, 128, 192, 256]))
+            helper = bool(rng.integers(0, 2))
+            fpt.set_launch(block, per_sm, max_blocks)
+            fpt.set_tail_helper(helper)
+            try:
+                out = run_gpu(w, n, check_every=K)
+            finally:
+                fpt.set_launch(0, 0, 0)
+                fpt.set_tail_helper(True)
+            assert all(np.array_equal(a, b) for a, b in zip(out, ref)), (block, per_sm, max_blocks, K, helper)
+
+
 # edge and degenerate cases
 def test_edge_cases():
     w = fpt.workload("c2")

@@ -32,6 +32,8 @@ def main():
     ap.add_argument("workloads", nargs="*", default=list(WORKLOADS))
     ap.add_argument("--k", default="0")
     ap.add_argument("--geoms", default="0x0,128x1,128x2,128x3,128x4,256x1,256x2")
+    ap.add_argument("--schedule", default="dynamic", choices=["dynamic", "static"],
+                    help="static = the split of the paper's Appendix A (lane j owns runs j, j+L, ...), for the scheduler A/B")
     args = ap.parse_args()
     ks = [int(x) for x in args.k.split(",")]
     geoms = [tuple(int(y) for y in g.split("x")) for g in args.geoms.split(",")]
@@ -43,6 +45,7 @@ def main():
         for k in ks:
             for block, per_sm in geoms:
                 fpt.set_launch(block, per_sm, 0)
+                fpt.set_schedule(args.schedule)
                 try:
                     prm = fpt.make_params(**dict(w["params"], check_every=k))
                     out = fpt._alloc_outputs(n)
@@ -58,13 +61,14 @@ def main():
                     st = fpt.last_stats()
                 finally:
                     fpt.set_launch(0, 0, 0)
+                    fpt.set_schedule("dynamic")
                 h = hashlib.md5(out[0].cpu().numpy().tobytes() + out[2].cpu().numpy().tobytes()).hexdigest()[:8]
                 ref = ref or h
                 sec = statistics.median(ms) * 1e-3
                 peak = peak32 if w["params"]["precision"] == "fp32" else peak64
                 print(f"{name:9s} K={st['check_every']:3d} block={st['block']:3d} per_sm={per_sm} grid={st['grid']:5d} ms={sec * 1e3:9.3f} "
                       f"steps/s={st['useful_steps'] / sec:.3e} frac={st['useful_steps'] / sec * w['n64_ref'] / peak:.3f} "
-                      f"lane_eff={st['lane_efficiency']:.3f} {h}{'' if h == ref else ' MISMATCH'}", flush=True)
+                      f"lane_eff={st['lane_efficiency']:.3f} runs_per_lane={n / (st['grid'] * st['block']):.1f} {h}{'' if h == ref else ' MISMATCH'}", flush=True)
 
 
 if __name__ == "__main__":

@@ -426,6 +426,37 @@ def test_random_geometries_poll_intervals_and_helper_settings_agree():
             assert all(np.array_equal(a, b) for a, b in zip(out, ref)), (block, per_sm, max_blocks, K, helper)
 
 
+def test_calls_can_be_captured_in_a_cuda_graph():
+    """fpt_simulate only enqueues stream-ordered work (pool allocation, memset, launch, copy, free), so a sequence of calls
+    can be captured once into a CUDA graph and replayed: same results as the eager calls, every replay."""
+    w = fpt.workload("c2", t_max=60.0)
+    n = 2048
+    p = fpt.make_params(**w["params"])
+    ref = fpt.simulate(p, n, 7, w["t_max"])
+    torch.cuda.synchronize()
+    ref = tuple(t.clone() for t in ref)
+    out = fpt.binding._alloc_outputs(n)
+    out2 = fpt.binding._alloc_outputs(n)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):                       # warm-up on the capture stream (lazy module loading is not capturable)
+        fpt.simulate(p, n, 7, w["t_max"], out=out, stream=side)
+    torch.cuda.current_stream().wait_stream(side)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        cs = torch.cuda.current_stream()
+        fpt.simulate(p, n, 7, w["t_max"], out=out, stream=cs)
+        fpt.simulate(p, n, 8, w["t_max"], out=out2, stream=cs)
+    for _ in range(3):
+        for t in out + out2:
+            t.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert all(torch.equal(a, b) for a, b in zip(out, ref))
+        assert not torch.equal(out2[0], ref[0]) and int((out2[2] == 0).sum()) > 0
+
+
 # edge and degenerate cases
 def test_edge_cases():
     w = fpt.workload("c2")

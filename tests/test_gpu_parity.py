@@ -8,6 +8,7 @@ seeded inputs.  Bars (BASELINE.json north_star, written out here):
   * distributions: two-sample KS p > 0.01 between GPU ids and an INDEPENDENT oracle sample (other ids).
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -402,7 +403,7 @@ def test_concurrent_streams_and_host_threads():
 
 
 def test_random_geometries_poll_intervals_and_helper_settings_agree():
-    """Stress of the scheduling machinery (refill, parking / adoption, tail helper, lobby): 40 random launch geometries,
+    """Stress of the scheduling machinery (refill, parking / adoption, tail helper, lobby): 40 (FPT_STRESS_TRIALS) random launch geometries,
     poll intervals and helper settings on workloads with escaped AND censored trajectories must all give the outputs of
     the first run, bit for bit -- the outputs are a function of (params, seed, id) only."""
     rng = np.random.default_rng(99)
@@ -410,7 +411,7 @@ def test_random_geometries_poll_intervals_and_helper_settings_agree():
                  (fpt.workload("c4", nu=2e-4, t_max=2220.0), 3000)]:
         ref = run_gpu(w, n)
         assert 0 < np.sum(ref[2] == 1) < n and np.sum(ref[2] == 0) > 0
-        for trial in range(40):
+        for trial in range(int(os.environ.get("FPT_STRESS_TRIALS", "40"))):
             block = int(rng.choice([32, 64, 96, 128, 160, 192, 224, 256]))
             per_sm = int(rng.choice([0, 1, 2, 3]))
             max_blocks = int(rng.choice([0, 1, 3, 7, 20, 148]))

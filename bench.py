@@ -306,7 +306,7 @@ def main():
                 f"{'FFMA' if fp32 else 'DFMA'} chains measured live by fpt_fp{'32' if fp32 else '64'}_peak after 1 s of load "
                 f"(SM clock seen {clk_hz / 1e6:.0f} MHz); MEASURED_PEAKS.json has no {'FP32' if fp32 else 'FP64'} figure",
         "hbm_bytes_per_step_algorithmic": n_traj * 20,
-        "fp64_instr_per_step_in_sass": {"c1": 31.4, "c2": 73.4, "c3": 75.4, "c5": 48.4}.get(args.workload),
+        "fp64_instr_per_step_in_sass": {"c1": 30.9, "c2": 72.9, "c3": 74.9, "c5": 47.9}.get(args.workload),
     }
 
     if rank == 0 and world == 1 and not args.no_extra:

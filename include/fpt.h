@@ -24,7 +24,8 @@
  *     No exceptions, no errno, no printing.  fpt_strerror() gives a static string (for FPT_E_CUDA: the CUDA error
  *     string of the most recent failure on the calling thread).
  *   - Determinism: per-trajectory outputs are a pure function of (params, seed, trajectory id); they do not depend on
- *     launch geometry, on check_every, on the GPU, or on which lane integrated which trajectory.
+ *     launch geometry, on check_every, on the scheduler and tail-helper settings, on the GPU, or on which lane
+ *     integrated which trajectory.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns FPT_E_CUDA.
  */
 #ifndef FPT_B200_H_

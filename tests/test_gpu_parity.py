@@ -558,3 +558,25 @@ def test_config1_distribution_vs_inverse_gaussian():
     cdf = lambda t: sst.invgauss.cdf(t, mu=(a / mu) / lam, scale=lam)
     assert sst.kstest(f, cdf).pvalue > 0.01
     assert abs(f.mean() - a / mu) < 5 * math.sqrt(0.2 / 20000)
+
+
+def test_distributions_ks_against_independent_oracle_samples():
+    """north_star: "the distributions must pass a two-sample KS test at p > 0.01" -- GPU ids [0, n) against an INDEPENDENT
+    oracle sample (other ids; identical ids would make the test vacuous) on the families of configs 3, 4 and 5; and the fp32
+    path against an fp64 oracle sample of the same physics (the paper's own CPU-double vs GPU-single check)."""
+    from scipy import stats as sst
+    n = 3000
+    w3 = fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3)
+    g3 = run_gpu(w3, n)[1]
+    assert sst.ks_2samp(g3, run_oracle(w3, n, first_id=10**7)["gamma"]).pvalue > 0.01
+    w5 = fpt.workload("c5", temperature=0.12, t_max=1e5)
+    f5, _, s5 = run_gpu(w5, n)
+    o5 = run_oracle(w5, n, first_id=10**7)
+    assert np.all(s5 == 0) and np.all(o5["status"] == 0)
+    assert sst.ks_2samp(f5, o5["fpt"]).pvalue > 0.01
+    w4 = fpt.workload("c4", nu=5e-5, t_max=0.55 / 5e-5)
+    g4 = run_gpu(w4, n)[1]
+    assert sst.ks_2samp(g4, run_oracle(w4, n, first_id=10**7)["gamma"]).pvalue > 0.01
+    w4d = fpt.workload("c4", nu=5e-5, t_max=0.55 / 5e-5, precision="fp64")
+    assert sst.ks_2samp(g4, run_oracle(w4d, n, first_id=2 * 10**7)["gamma"]).pvalue > 0.01
+

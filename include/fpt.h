@@ -19,13 +19,15 @@
  *     ends in _host.  `p` is HOST memory, read during the call only.  The library keeps no pointer after returning.
  *   - Calls enqueue work on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default stream) of the
  *     CURRENT device and return without synchronising; outputs are valid once the stream has been synchronised.
- *     (_host and fpt_last_stats / fpt_*_peak synchronise before returning.)
+ *     (_host and fpt_last_stats synchronise before returning.)
  *   - Return value: FPT_OK, or a negative code.  On FPT_E_INVALID nothing has been enqueued or written.
  *     No exceptions, no errno, no printing.  fpt_strerror() gives a static string (for FPT_E_CUDA: the CUDA error
  *     string of the most recent failure on the calling thread).
  *   - Determinism: per-trajectory outputs are a pure function of (params, seed, trajectory id); they do not depend on
- *     launch geometry, on check_every, on the scheduler and tail-helper settings, on the GPU, or on which lane
- *     integrated which trajectory.
+ *     launch geometry, on check_every, on any field of fpt_launch_opts (scheduler, tail helper, specialised kernel), on
+ *     the GPU, or on which lane integrated which trajectory.
+ *   - No state outside a call: the library owns a per-device memory pool and stream pool (caches), nothing a result or a
+ *     later call depends on.  Test hooks and the pipe-peak microbenchmarks live in fpt_dbg.h.
  *   - There is no CPU fallback: without a CUDA device every compute entry point returns FPT_E_CUDA.
  */
 #ifndef FPT_B200_H_
@@ -72,7 +74,8 @@ typedef struct fpt_params {
   uint64_t first_id;     /* trajectory id of element 0 of the outputs (sharding); the Philox stream is keyed by (seed, id) */
 } fpt_params;
 
-/* Counters of the most recent fpt_simulate* call on the current device (fpt_last_stats). */
+/* Counters and launch geometry of ONE fpt_simulate* call, written by the call's own kernels (stream ordered) into the
+ * caller's device block (fpt_simulate_ex: d_stats) -- nothing is shared between calls. */
 typedef struct fpt_stats {
   uint64_t n_traj;             /* trajectories processed                                                  */
   uint64_t n_escaped, n_censored, n_nan;
@@ -82,11 +85,49 @@ typedef struct fpt_stats {
   uint64_t n_cap;              /* step cap used = nearbyint(t_max/dt)                                     */
   int32_t  grid, block;        /* launch geometry used                                                    */
   int32_t  check_every;        /* effective K                                                             */
-  int32_t  reserved;
+  int32_t  kernel;             /* FPT_KERNEL_FILL | _PERSISTENT | _SPECIALISED: which kernel integrated    */
   uint64_t migrations;         /* trajectories parked by a sparse warp and adopted by another (drain-phase compaction) */
-  uint64_t helper_lane_steps;  /* 32 * (steps whose normals a tail-helper warp generated for its block's last live warp);
+  uint64_t helper_lane_steps;  /* 32 * (steps whose normals a tail-helper or producer warp generated for another warp);
                                   NOT part of issued_lane_steps                                            */
 } fpt_stats;
+
+#define FPT_KERNEL_FILL        0   /* every trajectory decided at k = 0 (phi0 >= threshold) or by n_cap == 0: no integration */
+#define FPT_KERNEL_PERSISTENT  1   /* every warp generates its own normals and integrates (filled GPU)                         */
+#define FPT_KERNEL_SPECIALISED 2   /* consumer warps integrate, producer warps generate their normals (under-filled GPU)       */
+
+/* Launch options of ONE call (fpt_simulate_ex).  Results never depend on any of them; only the time does.  A zeroed
+ * struct (or a NULL pointer) means the library's defaults. */
+#define FPT_SCHEDULE_DYNAMIC 0
+#define FPT_SCHEDULE_STATIC  1
+typedef struct fpt_launch_opts {
+  int32_t block;          /* persistent kernel: threads per block, a multiple of 32 in 32..256; 0 = default           */
+  int32_t blocks_per_sm;  /* persistent kernel: resident blocks per SM, 0 = default (occupancy / workload heuristic)   */
+  int32_t max_blocks;     /* cap on the grid, 0 = none                                                                 */
+  int32_t schedule;       /* FPT_SCHEDULE_DYNAMIC (default): a finished lane takes the next id from a global counter at
+                             once and sparse warps hand their trajectories over in the drain phase;
+                             FPT_SCHEDULE_STATIC: the static split analysed in the paper's Appendix A:
+                             lane j of L owns runs j, j+L, j+2L, ...; nothing is handed over, a warp lives as long as its
+                             slowest lane (with one run per lane: the paper's own kernel).  It exists to
+                             measure what the dynamic scheduler buys (fpt_stats lane efficiency against Eq. (A.5)).       */
+  int32_t tail_helper;    /* 0 = default (on), 1 = on, -1 = off.  Persistent kernel: when a block is down to one live warp
+                             and nothing is parked, the block's retired warps generate that warp's normals (Philox +
+                             Box-Muller) one chunk ahead into shared memory and the survivor only integrates.  Engages only
+                             in blocks of >= 3 warps, with a poll interval that is a multiple of 64 steps (fp64) / 32 (fp32),
+                             and for drifts with a sine (amp != 0).                                                      */
+  int32_t specialise;     /* 0 = automatic (the specialised kernel when the job cannot fill the GPU: fewer than two
+                             trajectories-in-flight warps per SM sub-partition), 1 = always, -1 = never.  Needs amp != 0 and
+                             the dynamic schedule; otherwise the persistent kernel runs.                                  */
+  int32_t consumers;      /* specialised kernel: consumer warps per block, 1..4 (0 = default)                           */
+  int32_t producers;      /* specialised kernel: producer warps per consumer, 1..3 (0 = default)                        */
+} fpt_launch_opts;
+
+/* Fused histogram request of fpt_simulate_ex (as fpt_simulate_hist). */
+typedef struct fpt_hist {
+  int32_t   of;           /* 0 = bias at escape, 1 = escape time */
+  int32_t   nbins;        /* 1..8192 */
+  double    lo, hi;
+  uint64_t* out_counts;   /* device, nbins + 2, ACCUMULATED into */
+} fpt_hist;
 
 /* Integrate trajectories id = first_id .. first_id+n_traj-1 until first passage or the cap n_cap = nearbyint(t_max/dt).
  *   out_fpt[i]     (double, required) k_esc*dt; -1.0 if censored; NaN if status 2
@@ -105,6 +146,16 @@ int fpt_simulate(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_ma
 int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
                       double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
                       int32_t hist_of, double lo, double hi, int32_t nbins, uint64_t* out_counts, void* cuda_stream);
+
+/* The general entry point: fpt_simulate / fpt_simulate_hist with per-call launch options and per-call statistics, and
+ * no state outside the call.  hist: NULL = no histogram.  opts: NULL = defaults.  d_stats (DEVICE memory, may be NULL):
+ * receives this call's fpt_stats, written stream-ordered after the integration (valid once cuda_stream has been
+ * synchronised).  Calls from any number of host threads on any number of streams are independent.
+ * Additional FPT_E_INVALID: a bad field of opts (block not a multiple of 32 in 32..256, negative counts, unknown schedule,
+ * consumers > 4, producers > 3) or of hist (as fpt_simulate_hist). */
+int fpt_simulate_ex(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
+                    double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
+                    const fpt_hist* hist, const fpt_launch_opts* opts, fpt_stats* d_stats, void* cuda_stream);
 
 /* Histogram of values[i] over the entries with status[i] == 0 (status may be NULL: all entries):
  *   b = floor((x - lo) * (nbins/(hi-lo))) in fp64, the scale computed once; b < 0 -> under, b >= nbins -> over (x == hi is
@@ -130,66 +181,25 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
  * long as its longest trajectory), forked from and joined back into cuda_stream, so to the caller this is one
  * asynchronous call like fpt_simulate.  Each result is bit-identical to a separate fpt_simulate of that set.
  * sets and t_max are host arrays read during the call.  FPT_E_INVALID as fpt_simulate for any set (nothing is
- * launched then), or NULL sets / t_max, n_sets < 0.  fpt_last_stats afterwards describes one of the sets. */
+ * launched then), or NULL sets / t_max, n_sets < 0.  fpt_last_stats afterwards describes the last set. */
 int fpt_simulate_sweep(const fpt_params* sets, int32_t n_sets, int64_t n_per_set, uint64_t seed, const double* t_max,
                        double* out_fpt, double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream);
 
-/* Launch geometry override for subsequent fpt_simulate* calls of this process (results never depend on it):
- * block = threads per block (multiple of 32, 32..256; 0 = default), blocks_per_sm (0 = default from the occupancy
- * calculator), max_blocks (0 = no extra cap).  FPT_E_INVALID on a bad value. */
-int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks);
+/* DEPRECATED conveniences, kept for one release: defaults for the calls that take no fpt_launch_opts (fpt_simulate,
+ * fpt_simulate_hist, fpt_simulate_host, fpt_simulate_sweep) made afterwards BY THE CALLING THREAD (thread-local; no
+ * process-wide state).  New code passes fpt_launch_opts to fpt_simulate_ex.  FPT_E_INVALID on a bad value. */
+int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks);   /* fields of the same names          */
+int fpt_set_schedule(int32_t schedule);                                         /* FPT_SCHEDULE_*                    */
+int fpt_set_tail_helper(int32_t on);                                            /* 1 on (default), 0 off             */
+int fpt_set_specialise(int32_t specialise, int32_t consumers, int32_t producers);
 
-/* Scheduler of subsequent fpt_simulate* calls of this process (results never depend on it; only the time does):
- *   FPT_SCHEDULE_DYNAMIC (default) a finished lane takes the next id from a global counter at once, and
- *                        sparse warps hand their trajectories over in the drain phase;
- *   FPT_SCHEDULE_STATIC  the static split analysed in the paper's Appendix A: lane j of L owns runs
- *                        j, j+L, j+2L, ...; nothing is handed over, a warp lives as long as its slowest lane.  With one
- *                        run per lane this is the paper's own kernel (one thread per realisation).  It exists
- *                        to measure what the dynamic scheduler buys (fpt_stats lane efficiency against Eq. (A.5)). */
-#define FPT_SCHEDULE_DYNAMIC 0
-#define FPT_SCHEDULE_STATIC  1
-int fpt_set_schedule(int32_t schedule);
-
-/* Tail helper (default on; results never depend on it): when a block is down to one live warp and nothing is parked, a
- * retired warp of the block generates that warp's normals (Philox + Box-Muller) one chunk ahead into shared memory and the
- * survivor only integrates, which shortens the time a launch waits for its longest trajectories.  Needs blocks of at least
- * two warps and a poll interval that is a multiple of 32 steps; otherwise it stays off by itself. */
-int fpt_set_tail_helper(int32_t on);
-
-/* Synchronises the current device and returns the counters of the most recent fpt_simulate* call on it. */
+/* DEPRECATED: synchronises the current device and returns the fpt_stats of the most recent fpt_simulate* call the
+ * CALLING THREAD made on it (a zeroed struct if it made none).  Concurrent callers pass their own d_stats to
+ * fpt_simulate_ex instead. */
 int fpt_last_stats(fpt_stats* out);
-
-/* Roofline denominators measured live: a kernel of independent DFMA (fp64) or FFMA (fp32) chains on every SM, run
- * repeatedly for about `seconds`; *inst_per_s = thread-instructions per second, *sm_clock_hz = SM clock seen by the
- * kernel (clock64 ticks / elapsed time; may be NULL). */
-int fpt_fp64_peak(double seconds, double* inst_per_s, double* sm_clock_hz);
-int fpt_fp32_peak(double seconds, double* inst_per_s, double* sm_clock_hz);
 
 const char* fpt_strerror(int code);
 int fpt_version(void);   /* 10000*major + 100*minor + patch */
-
-/* ---- test hooks: the device functions of the hot path, exposed one by one so that tests can compare bits with the
- * oracle.  All pointers are device memory; work is enqueued on cuda_stream. ---- */
-/* out[4*i..4*i+3] = Philox4x32-10 block `block` of stream (seed, id0+i) */
-int fpt_dbg_philox(uint64_t seed, uint64_t id0, int64_t n_ids, uint64_t block, uint32_t* out, void* cuda_stream);
-/* normals of blocks b0..b0+nblocks-1 of stream (seed, id): fp64 2 per block (z_a, z_b); fp32 4 per block */
-int fpt_dbg_normals_f64(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, double* out, void* cuda_stream);
-int fpt_dbg_normals_f32(uint64_t seed, uint64_t id, uint64_t b0, int64_t nblocks, float* out, void* cuda_stream);
-/* elementwise: which = 0 sin_drift(x), 1 neg2log(x) (x in (0,1)) */
-int fpt_dbg_unary_f64(int32_t which, const double* x, double* y, int64_t n, void* cuda_stream);
-int fpt_dbg_unary_f32(int32_t which, const float* x, float* y, int64_t n, void* cuda_stream);
-/* cos, sin of the Box-Muller angle from the raw 64-bit (fp64) / 32-bit (fp32) word */
-int fpt_dbg_sincos_f64(const uint64_t* Y, double* c, double* s, int64_t n, void* cuda_stream);
-int fpt_dbg_sincos_f32(const uint32_t* o, float* c, float* s, int64_t n, void* cuda_stream);
-/* the guard-free division / square-root sequences of csrc/fpt_math.cuh against nvcc's IEEE builtins, on operands drawn
- * from the real pipeline (n_threads streams, a multiple of 128, x blocks_per_thread Philox blocks each):
- * out4[0..3] += number of bit mismatches {fp64 div, fp64 sqrt, fp32 div, fp32 sqrt} (device, uint64, caller zeroes). */
-int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t blocks_per_thread, uint64_t* out4,
-                      void* cuda_stream);
-/* one trajectory (id) with its states recorded: trace_phi[k], trace_v[k] for k = 0..min(k_end, trace_len-1) (as double),
- * out_status[0], out_k_end[0]; entries past k_end are left untouched. */
-int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len,
-                  double* trace_phi, double* trace_v, int32_t* out_status, uint64_t* out_k_end, void* cuda_stream);
 
 #ifdef __cplusplus
 }

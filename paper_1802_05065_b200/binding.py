@@ -16,6 +16,7 @@ MODEL = {"overdamped": 0, "underdamped": 1}
 SCHEME = {"em": 0, "heun": 1}
 PRECISION = {"fp64": 0, "fp32": 1}
 HIST_OF = {"gamma": 0, "fpt": 1}
+SCHEDULE = {"dynamic": 0, "static": 1}
 
 
 class FptError(RuntimeError):
@@ -35,13 +36,26 @@ class FptStats(C.Structure):
     _fields_ = [("n_traj", C.c_uint64), ("n_escaped", C.c_uint64), ("n_censored", C.c_uint64), ("n_nan", C.c_uint64),
                 ("useful_steps", C.c_uint64), ("issued_lane_steps", C.c_uint64), ("refill_atomics", C.c_uint64),
                 ("n_cap", C.c_uint64), ("grid", C.c_int32), ("block", C.c_int32), ("check_every", C.c_int32),
-                ("reserved", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64)]
+                ("kernel", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64)]
 
     def as_dict(self):
-        d = {k: int(getattr(self, k)) for k, _ in self._fields_ if k != "reserved"}
+        d = {k: int(getattr(self, k)) for k, _ in self._fields_}
         d["lane_efficiency"] = d["useful_steps"] / d["issued_lane_steps"] if d["issued_lane_steps"] else None
         return d
 
+
+class FptLaunchOpts(C.Structure):
+    """struct fpt_launch_opts of include/fpt.h (32 bytes); all zero = the library's defaults."""
+    _fields_ = [("block", C.c_int32), ("blocks_per_sm", C.c_int32), ("max_blocks", C.c_int32), ("schedule", C.c_int32),
+                ("tail_helper", C.c_int32), ("specialise", C.c_int32), ("consumers", C.c_int32), ("producers", C.c_int32)]
+
+
+class FptHist(C.Structure):
+    """struct fpt_hist of include/fpt.h."""
+    _fields_ = [("of", C.c_int32), ("nbins", C.c_int32), ("lo", C.c_double), ("hi", C.c_double), ("out_counts", C.c_void_p)]
+
+
+KERNEL = {0: "fill", 1: "persistent", 2: "specialised"}
 
 _lib = None
 
@@ -49,6 +63,8 @@ _SIGNATURES = {
     "fpt_simulate": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p],
     "fpt_simulate_hist": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
+    "fpt_simulate_ex": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                        C.POINTER(FptHist), C.POINTER(FptLaunchOpts), C.c_void_p, C.c_void_p],
     "fpt_histogram": [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_simulate_host": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p],
@@ -57,6 +73,7 @@ _SIGNATURES = {
     "fpt_set_launch": [C.c_int32, C.c_int32, C.c_int32],
     "fpt_set_schedule": [C.c_int32],
     "fpt_set_tail_helper": [C.c_int32],
+    "fpt_set_specialise": [C.c_int32, C.c_int32, C.c_int32],
     "fpt_last_stats": [C.POINTER(FptStats)],
     "fpt_fp64_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
     "fpt_fp32_peak": [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)],
@@ -70,6 +87,7 @@ _SIGNATURES = {
     "fpt_dbg_sincos_f64": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
     "fpt_dbg_sincos_f32": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
     "fpt_dbg_selfcheck": [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p],
+    "fpt_dbg_set_helper_seq0": [C.c_uint64],
     "fpt_dbg_trace": [C.POINTER(FptParams), C.c_uint64, C.c_uint64, C.c_double, C.c_int64, C.c_void_p, C.c_void_p,
                       C.c_void_p, C.c_void_p, C.c_void_p],
 }
@@ -133,6 +151,46 @@ def simulate(params: FptParams, n_traj: int, seed: int, t_max: float, out=None, 
     return fpt, gam, st
 
 
+def launch_opts(block=0, blocks_per_sm=0, max_blocks=0, schedule="dynamic", tail_helper=None, specialise=None, consumers=0,
+                producers=0) -> FptLaunchOpts:
+    """fpt_launch_opts.  tail_helper / specialise: None = the library's default, True = on / always, False = off / never."""
+    tri = lambda v: 0 if v is None else (1 if v else -1)
+    sch = SCHEDULE[schedule] if isinstance(schedule, str) else int(schedule)
+    return FptLaunchOpts(block, blocks_per_sm, max_blocks, sch, tri(tail_helper), tri(specialise), consumers, producers)
+
+
+def alloc_stats(n=1):
+    """Device memory for n fpt_stats blocks (the d_stats argument of simulate_ex)."""
+    import torch
+    return torch.zeros(n * C.sizeof(FptStats), dtype=torch.uint8, device=torch.device("cuda", torch.cuda.current_device()))
+
+
+def read_stats(d_stats, i=0) -> dict:
+    """The i-th fpt_stats block of `d_stats` as a dict (synchronises through the device-to-host copy)."""
+    raw = d_stats[i * C.sizeof(FptStats):(i + 1) * C.sizeof(FptStats)].cpu().numpy().tobytes()
+    return FptStats.from_buffer_copy(raw).as_dict()
+
+
+def simulate_ex(params: FptParams, n_traj: int, seed: int, t_max: float, hist=None, opts=None, stats=None, out=None,
+                stream=None):
+    """fpt_simulate_ex.  hist = (hist_of, lo, hi, nbins, counts CUDA tensor) or None; opts = FptLaunchOpts or None; stats =
+    a uint8 CUDA tensor from alloc_stats() (or a (tensor, index) pair) that receives this call's fpt_stats, or None.
+    Returns (fpt, gamma, status).  Asynchronous."""
+    fpt, gam, st = out if out is not None else _alloc_outputs(n_traj)
+    h = None
+    if hist is not None:
+        of, lo, hi, nb, counts = hist
+        h = FptHist(HIST_OF[of] if isinstance(of, str) else int(of), nb, lo, hi, counts.data_ptr())
+    sp = C.c_void_p(0)
+    if stats is not None:
+        t, i = stats if isinstance(stats, tuple) else (stats, 0)
+        sp = C.c_void_p(t.data_ptr() + i * C.sizeof(FptStats))
+    _check(lib().fpt_simulate_ex(C.byref(params), n_traj, seed, t_max, _ptr(fpt), _ptr(gam), _ptr(st),
+                                 C.byref(h) if h is not None else None, C.byref(opts) if opts is not None else None, sp,
+                                 _stream(stream)), "fpt_simulate_ex")
+    return fpt, gam, st
+
+
 def simulate_hist(params: FptParams, n_traj: int, seed: int, t_max: float, lo: float, hi: float, nbins: int,
                   hist_of="gamma", counts=None, out=None, stream=None):
     """fpt_simulate_hist.  `counts` (uint64-as-int64 CUDA tensor of nbins+2) is accumulated into; zeros when None."""
@@ -191,9 +249,6 @@ def set_launch(block=0, blocks_per_sm=0, max_blocks=0):
     _check(lib().fpt_set_launch(block, blocks_per_sm, max_blocks), "fpt_set_launch")
 
 
-SCHEDULE = {"dynamic": 0, "static": 1}
-
-
 def set_schedule(schedule="dynamic"):
     """fpt_set_schedule: "dynamic" (refill + drain compaction, default) or "static" (Appendix A's split, for the A/B)."""
     v = SCHEDULE[schedule] if isinstance(schedule, str) else int(schedule)
@@ -202,6 +257,12 @@ def set_schedule(schedule="dynamic"):
 
 def set_tail_helper(on=True):
     _check(lib().fpt_set_tail_helper(1 if on else 0), "fpt_set_tail_helper")
+
+
+def set_specialise(specialise=None, consumers=0, producers=0):
+    """fpt_set_specialise: None = automatic, True = always, False = never (thread-local default of the plain calls)."""
+    v = 0 if specialise is None else (1 if specialise else -1)
+    _check(lib().fpt_set_specialise(v, consumers, producers), "fpt_set_specialise")
 
 
 def last_stats() -> dict:
@@ -283,6 +344,10 @@ def dbg_selfcheck(seed, id0, n_threads, blocks_per_thread, stream=None):
     out = torch.zeros(4, dtype=torch.int64, device="cuda")
     _check(lib().fpt_dbg_selfcheck(seed, id0, n_threads, blocks_per_thread, _ptr(out), _stream(stream)), "fpt_dbg_selfcheck")
     return out
+
+
+def dbg_set_helper_seq0(seq0=0):
+    _check(lib().fpt_dbg_set_helper_seq0(seq0), "fpt_dbg_set_helper_seq0")
 
 
 def dbg_trace(params: FptParams, seed, tid, t_max, trace_len, stream=None):

@@ -34,8 +34,7 @@ def _nvcc() -> str:
 
 
 def _sources():
-    return [p for p in list(CSRC.iterdir()) + [INCLUDE / "fpt.h"]
-            if p.suffix in (".cu", ".cuh", ".h") and p.name != "fpt_microbench.cu"]
+    return [p for p in list(CSRC.iterdir()) + [INCLUDE / "fpt.h", INCLUDE / "fpt_dbg.h"] if p.suffix in (".cu", ".cuh", ".h")]
 
 
 def up_to_date() -> bool:
@@ -70,18 +69,5 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
-def build_microbench() -> Path:
-    """The stand-alone issue-rate microbenchmark of DESIGN.md section 9 (csrc/fpt_microbench.cu)."""
-    exe = HERE / "fpt_microbench"
-    cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", str(exe), str(CSRC / "fpt_microbench.cu")]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if r.returncode != 0:
-        raise RuntimeError(f"nvcc failed on fpt_microbench.cu:\n{r.stdout}\n{r.stderr}")
-    return exe
-
-
 if __name__ == "__main__":
-    if "--microbench" in sys.argv:
-        print(build_microbench())
-    else:
-        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,6 +1,9 @@
-// fpt_api.cu -- the C ABI of include/fpt.h: argument validation, the host-side derived constants,
-// launch geometry, the standalone histogram kernel, the roofline microbenchmarks and the test hooks.
+// fpt_api.cu -- the C ABI of include/fpt.h and include/fpt_dbg.h: argument validation, the host-side derived constants
+// (DESIGN.md 4.8), launch geometry and kernel choice, the standalone histogram kernel, the roofline microbenchmarks and the
+// test hooks.  Nothing a result or a later call depends on is kept between calls: launch options and statistics travel
+// with the call (fpt_launch_opts, d_stats); the library owns only caches (a memory pool and a stream pool per device).
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -8,6 +11,7 @@
 #include <vector>
 
 #include "../../include/fpt.h"
+#include "../../include/fpt_dbg.h"
 #include "fpt_inst.cuh"
 #include "fpt_integrator.cuh"
 
@@ -31,53 +35,65 @@ constexpr int kMaxDevices = 64;
 // default poll interval in steps: measured on B200, a poll costs about as much as 1.3 steps (the software pipeline of the
 // step loop drains and refills around it), so 64 (fp64) / 32 (fp32) steps keep it near 2 %; a finished lane idles K/2 steps
 constexpr int kDefaultK64 = 64, kDefaultK32 = 32;
+// specialised kernel (fpt_specialised.cuh): hand-over chunk = its poll interval; limits of fpt_launch_opts
+constexpr int kSpecChunk64 = 64, kSpecChunk32 = 32;
+constexpr int kSpecMaxConsumersHost = 4, kSpecMaxProducersHost = 3;
 
-struct LaunchCfg {
-  int block = 0, blocks_per_sm = 0, max_blocks = 0;
-  int schedule = 0;
-  int tail_helper = 1;
-};
-std::mutex g_mu;
-LaunchCfg g_cfg;
+// Defaults of the calls that take no fpt_launch_opts: per THREAD (the deprecated fpt_set_* shims write them).
+thread_local fpt_launch_opts t_opts = {};
+thread_local unsigned long long t_dbg_seq0 = 0;
 
 constexpr int kSweepStreams = 8;
+constexpr int kLastSlots = 256;   // ring of "last call" statistics blocks per device (fpt_last_stats shim)
 
-struct DeviceCtx {          // per device: the "last call" counters, and the stream pool of fpt_simulate_sweep
+struct DeviceCtx {          // per device: caches only
+  std::mutex mu;                 // serialises fpt_simulate_sweep's use of the stream pool
   cudaStream_t pool[kSweepStreams] = {};
-  cudaEvent_t pool_done[kSweepStreams] = {};
-  cudaEvent_t fork = nullptr;
   bool pool_ready = false;
   cudaMemPool_t mem = nullptr;   // the library's own stream-ordered pool: freed blocks stay cached across synchronisations
-  DevStats* d_last = nullptr;
-  fpt_stats host{};         // geometry etc. filled at launch, counters read back on demand
-  cudaStream_t last_stream = nullptr;
-  bool valid = false;
+  fpt_stats* d_last = nullptr;   // kLastSlots blocks; a call writes its statistics into slot (ticket % kLastSlots)
+  unsigned long long* d_ticket = nullptr;   // ticket of the call that owns each slot
+  std::atomic<unsigned long long> next_ticket{1};
   int sm_count = 0;
+  std::atomic<bool> ready{false};
 };
 DeviceCtx g_ctx[kMaxDevices];
+std::mutex g_init_mu;
 
-int device_ctx(DeviceCtx** out) {
+struct ThreadLast {         // ticket of the calling thread's most recent call, per device
+  unsigned long long ticket[kMaxDevices] = {};
+};
+thread_local ThreadLast t_last;
+
+int device_ctx(DeviceCtx** out, int* dev_out = nullptr) {
   int dev = 0;
   FPT_CUDA(cudaGetDevice(&dev));
   if (dev < 0 || dev >= kMaxDevices) return FPT_E_CUDA;
   DeviceCtx& c = g_ctx[dev];
-  if (!c.d_last) {
-    FPT_CUDA(cudaMalloc(&c.d_last, sizeof(DevStats)));
-    FPT_CUDA(cudaMemset(c.d_last, 0, sizeof(DevStats)));
-    FPT_CUDA(cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev));
-    // per-call workspaces come from a private memory pool that never trims (release threshold = max): with the device's
-    // default pool every stream synchronisation hands the memory back to the driver and the next call pays a real
-    // allocation (hundreds of microseconds, sometimes milliseconds) between the caller's event and the kernel launch
-    cudaMemPoolProps props{};
-    props.allocType = cudaMemAllocationTypePinned;
-    props.handleTypes = cudaMemHandleTypeNone;
-    props.location.type = cudaMemLocationTypeDevice;
-    props.location.id = dev;
-    FPT_CUDA(cudaMemPoolCreate(&c.mem, &props));
-    unsigned long long keep = ~0ull;
-    FPT_CUDA(cudaMemPoolSetAttribute(c.mem, cudaMemPoolAttrReleaseThreshold, &keep));
+  if (!c.ready.load(std::memory_order_acquire)) {
+    std::lock_guard<std::mutex> lk(g_init_mu);
+    if (!c.ready.load(std::memory_order_relaxed)) {
+      FPT_CUDA(cudaMalloc(&c.d_last, sizeof(fpt_stats) * kLastSlots));
+      FPT_CUDA(cudaMemset(c.d_last, 0, sizeof(fpt_stats) * kLastSlots));
+      FPT_CUDA(cudaMalloc(&c.d_ticket, sizeof(unsigned long long) * kLastSlots));
+      FPT_CUDA(cudaMemset(c.d_ticket, 0, sizeof(unsigned long long) * kLastSlots));
+      FPT_CUDA(cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev));
+      // per-call workspaces come from a private memory pool that never trims (release threshold = max): with the device's
+      // default pool every stream synchronisation hands the memory back to the driver and the next call pays a real
+      // allocation (hundreds of microseconds, sometimes milliseconds) between the caller's event and the kernel launch
+      cudaMemPoolProps props{};
+      props.allocType = cudaMemAllocationTypePinned;
+      props.handleTypes = cudaMemHandleTypeNone;
+      props.location.type = cudaMemLocationTypeDevice;
+      props.location.id = dev;
+      FPT_CUDA(cudaMemPoolCreate(&c.mem, &props));
+      unsigned long long keep = ~0ull;
+      FPT_CUDA(cudaMemPoolSetAttribute(c.mem, cudaMemPoolAttrReleaseThreshold, &keep));
+      c.ready.store(true, std::memory_order_release);
+    }
   }
   *out = &c;
+  if (dev_out) *dev_out = dev;
   return FPT_OK;
 }
 
@@ -96,6 +112,25 @@ int validate(const fpt_params* p, int64_t n_traj, double t_max) {
   if (!(p->dt > 0.0) || !(t_max > 0.0) || p->temperature < 0.0) return FPT_E_INVALID;
   if (p->model == 1 && p->alpha < 0.0) return FPT_E_INVALID;
   if (!(t_max / p->dt < 0x1p53)) return FPT_E_INVALID;
+  return FPT_OK;
+}
+
+int validate_opts(const fpt_launch_opts* o) {
+  if (!o) return FPT_OK;
+  if (o->block != 0 && (o->block < 32 || o->block > 256 || (o->block % 32) != 0)) return FPT_E_INVALID;
+  if (o->blocks_per_sm < 0 || o->blocks_per_sm > 64 || o->max_blocks < 0) return FPT_E_INVALID;
+  if (o->schedule != FPT_SCHEDULE_DYNAMIC && o->schedule != FPT_SCHEDULE_STATIC) return FPT_E_INVALID;
+  if (o->tail_helper < -1 || o->tail_helper > 1 || o->specialise < -1 || o->specialise > 1) return FPT_E_INVALID;
+  if (o->consumers < 0 || o->consumers > kSpecMaxConsumersHost || o->producers < 0 || o->producers > kSpecMaxProducersHost)
+    return FPT_E_INVALID;
+  return FPT_OK;
+}
+
+int validate_hist(const fpt_hist* h) {
+  if (!h) return FPT_OK;
+  if (!h->out_counts || h->nbins < 1 || h->nbins > kMaxFusedBins || !std::isfinite(h->lo) || !std::isfinite(h->hi) || !(h->hi > h->lo))
+    return FPT_E_INVALID;
+  if (h->of < 0 || h->of > 1) return FPT_E_INVALID;
   return FPT_OK;
 }
 
@@ -155,20 +190,59 @@ __global__ void fpt_fill_kernel(KParams P, int status, double fptv, double gam) 
   }
 }
 
+// The call's statistics: counters of its workspace + the geometry the host chose, written to the caller's block (may be
+// NULL) and to the call's slot of the per-device ring behind the deprecated fpt_last_stats.
+__global__ void fpt_export_stats_kernel(const DevStats* ws, fpt_stats geo, fpt_stats* user, fpt_stats* slot,
+                                        unsigned long long* slot_ticket, unsigned long long ticket) {
+  geo.n_escaped = ws->n_escaped;
+  geo.n_censored = ws->n_censored;
+  geo.n_nan = ws->n_nan;
+  geo.useful_steps = ws->useful_steps;
+  geo.issued_lane_steps = ws->issued_lane_steps;
+  geo.refill_atomics = ws->refill_atomics;
+  geo.migrations = ws->migrations;
+  geo.helper_lane_steps = ws->helper_lane_steps;
+  if (user) *user = geo;
+  *slot = geo;
+  *slot_ticket = ticket;
+}
+
+struct WsGuard {            // the per-call workspace goes back to the pool on every path, stream ordered
+  DevStats* ws = nullptr;
+  cudaStream_t stream = nullptr;
+  ~WsGuard() {
+    if (ws) (void)cudaFreeAsync(ws, stream);
+  }
+};
+
+// Opt in to more than 48 KB of shared memory when a launch needs it (fused histograms of many bins next to the drain pool
+// and the tail helper's buffer; the specialised kernel's hand-over rings).  FPT_E_INVALID when it cannot fit at all.
+int ensure_dynamic_smem(const void* fn, size_t dyn_bytes, int dev) {
+  cudaFuncAttributes a{};
+  FPT_CUDA(cudaFuncGetAttributes(&a, fn));
+  if (a.sharedSizeBytes + dyn_bytes <= 48 * 1024) return FPT_OK;
+  int optin = 0;
+  FPT_CUDA(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+  if (a.sharedSizeBytes + dyn_bytes > (size_t)optin) return FPT_E_INVALID;
+  if ((size_t)a.maxDynamicSharedSizeBytes >= dyn_bytes) return FPT_OK;
+  FPT_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_bytes));
+  return FPT_OK;
+}
+
 int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt, double* out_gamma,
-                  int32_t* out_status, bool with_hist, int32_t hist_of, double lo, double hi, int32_t nbins,
-                  uint64_t* out_counts, void* cuda_stream) {
+                  int32_t* out_status, const fpt_hist* hist, const fpt_launch_opts* opts_in, fpt_stats* d_stats,
+                  void* cuda_stream) {
   int rc = validate(p, n_traj, t_max);
   if (rc != FPT_OK) return rc;
   if (n_traj > 0 && (!out_fpt || !out_status)) return FPT_E_INVALID;   // empty outputs may be NULL
-  if (with_hist) {
-    if (!out_counts || nbins < 1 || nbins > kMaxFusedBins || !std::isfinite(lo) || !std::isfinite(hi) || !(hi > lo)) return FPT_E_INVALID;
-    if (hist_of < 0 || hist_of > 1) return FPT_E_INVALID;
-  }
+  if ((rc = validate_hist(hist)) != FPT_OK) return rc;
+  if ((rc = validate_opts(opts_in)) != FPT_OK) return rc;
   if (n_traj == 0) return FPT_OK;
+  const fpt_launch_opts cfg = opts_in ? *opts_in : t_opts;
   cudaStream_t stream = (cudaStream_t)cuda_stream;
   DeviceCtx* ctx = nullptr;
-  rc = device_ctx(&ctx);
+  int dev = 0;
+  rc = device_ctx(&ctx, &dev);
   if (rc != FPT_OK) return rc;
 
   KParams P;
@@ -177,29 +251,29 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
   P.out_fpt = out_fpt;
   P.out_gamma = out_gamma;
   P.out_status = out_status;
+  P.dbg_seq0 = t_dbg_seq0;
+  const bool with_hist = hist != nullptr;
   if (with_hist) {
-    P.hist_of = hist_of;
-    P.nbins = nbins;
-    P.hist_lo = lo;
-    P.hist_scale = (double)nbins / (hi - lo);
-    P.out_counts = (unsigned long long*)out_counts;
+    P.hist_of = hist->of;
+    P.nbins = hist->nbins;
+    P.hist_lo = hist->lo;
+    P.hist_scale = (double)hist->nbins / (hist->hi - hist->lo);
+    P.out_counts = (unsigned long long*)hist->out_counts;
   }
-  DevStats* ws = nullptr;
-  FPT_CUDA(cudaMallocFromPoolAsync(&ws, sizeof(DevStats), ctx->mem, stream));
+  WsGuard guard;
+  guard.stream = stream;
+  FPT_CUDA(cudaMallocFromPoolAsync(&guard.ws, sizeof(DevStats), ctx->mem, stream));
+  DevStats* ws = guard.ws;
   FPT_CUDA(cudaMemsetAsync(ws, 0, sizeof(DevStats), stream));
   P.ws = ws;
 
-  LaunchCfg cfg;
-  {
-    std::lock_guard<std::mutex> lk(g_mu);
-    cfg = g_cfg;
-  }
-  int grid = 1, block = 128;
+  int grid = 1, block = 128, kernel = FPT_KERNEL_FILL;
   const bool fp32 = p->precision == FPT_PREC_FP32;
+  const int sms = ctx->sm_count;
   const bool at_once_escaped = fp32 ? !((float)p->phi0 < (float)p->threshold) : !(p->phi0 < p->threshold);
   if (at_once_escaped || P.n_cap == 0) {
     block = 256;
-    grid = (int)std::min<int64_t>((n_traj + block - 1) / block, 148 * 8);
+    grid = (int)std::min<int64_t>((n_traj + block - 1) / block, (int64_t)sms * 8);
     const int status = at_once_escaped ? kStatusEscaped : kStatusCensored;
     const double fptv = at_once_escaped ? 0.0 : -1.0;
     const double gam = std::fma(P.dgamma, at_once_escaped ? 0.0 : (double)P.n_cap, P.gamma0);
@@ -207,74 +281,108 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     FPT_CUDA(cudaGetLastError());
   } else {
     const bool amp = p->amp != 0.0, ramp = p->nu != 0.0;
-    const void* fn = fp32 ? persistent_kernel_f32(p->model, p->scheme, amp, ramp)
-                          : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
-    const size_t smem = with_hist ? (size_t)(nbins + 2) * sizeof(unsigned int) : 0;
-    const int sms = ctx->sm_count;
-    auto max_blocks_per_sm = [&](int blk, int* out) -> cudaError_t {
-      return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, fn, blk, smem);
-    };
+    const size_t hist_bytes = with_hist ? (size_t)(hist->nbins + 2) * sizeof(unsigned int) : 0;
+    const long long unit = 128LL * sms;                         // one warp per SM sub-partition everywhere
+    // ---- which kernel.  The specialised kernel (consumers integrate, producers generate the normals) is for launches
+    // that cannot fill the GPU: with fewer than two warps of trajectories in flight per sub-partition a warp advances at
+    // the latency of its own instruction stream, and splitting that stream over warps shortens it.  Constant bias: the
+    // persistent kernel would keep n_traj / 5 trajectories in flight (below); ramped: all of them.
+    const bool explicit_geometry = cfg.block > 0 || cfg.blocks_per_sm > 0;
+    const long long in_flight = ramp ? n_traj : n_traj / 5;
+    const bool spec = amp && cfg.schedule == FPT_SCHEDULE_DYNAMIC && cfg.specialise >= 0 &&
+                      (cfg.specialise == 1 || (!explicit_geometry && in_flight < 2 * unit));
+    const void* fn = nullptr;
+    size_t smem = hist_bytes;
     long long blocks = 0;
-    if (cfg.block > 0 || cfg.blocks_per_sm > 0) {
-      // explicit geometry (fpt_set_launch): block x min(blocks_per_sm, occupancy limit) per SM
-      block = cfg.block > 0 ? cfg.block : 128;
+    if (spec) {
+      size_t chan = 0;
+      fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &chan) : specialised_kernel_f64(p->model, p->scheme, ramp, &chan);
+      int NC = cfg.consumers > 0 ? cfg.consumers : 4;
+      const int NP = cfg.producers > 0 ? cfg.producers : 2;
+      // few trajectories: fewer consumers per block, so that every SM gets some
+      while (cfg.consumers == 0 && NC > 1 && (long long)(NC - 1) * 32 * sms >= n_traj) --NC;
+      P.spec_consumers = NC;
+      P.spec_producers = NP;
+      P.K = fp32 ? kSpecChunk32 : kSpecChunk64;                   // one poll per hand-over chunk
+      block = 32 * NC * (1 + NP);
+      smem = (size_t)NC * chan + hist_bytes;
+      rc = ensure_dynamic_smem(fn, smem, dev);
+      if (rc != FPT_OK) return rc;
       int per_sm = 0;
-      FPT_CUDA(max_blocks_per_sm(block, &per_sm));
+      FPT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, smem));
       if (per_sm < 1) return FPT_E_CUDA;
-      if (cfg.blocks_per_sm > 0) per_sm = std::min(per_sm, cfg.blocks_per_sm);
+      per_sm = cfg.blocks_per_sm > 0 ? std::min(per_sm, cfg.blocks_per_sm) : 1;
       blocks = (long long)per_sm * sms;
+      const long long needed = (n_traj + 32LL * NC - 1) / (32LL * NC);
+      if (blocks > needed) blocks = needed;
+      kernel = FPT_KERNEL_SPECIALISED;
     } else {
-      // Default geometry.  Resident lanes = n_traj / R, at least one warp per SM sub-partition (128 lanes per SM) and at
-      // most what the registers allow.  R = 1 for a ramped bias (nu != 0: switching happens in a narrow window, all
-      // trajectories are about equally long, so throughput is everything); R = 5 for a constant bias (escape is a
-      // Poisson process, lengths are exponential: a launch lasts at least as long as its longest trajectory, and that
-      // one runs fastest when few warps share its SM sub-partition; the refills keep the lanes busy meanwhile).
-      const long long R = ramp ? 1 : 5;
-      const long long unit = 128LL * sms;                       // one warp per sub-partition everywhere
-      // ramped: round UP, so that a job that fits resident at once runs as one wave (C4: 65536 equal-length trajectories
-      // on 4 x 128 lanes per SM, not 3 x 128 plus a straggler wave); constant bias: round down, more refills per lane
-      long long units = ramp ? (n_traj + unit - 1) / unit : n_traj / (R * unit);
-      if (n_traj >= unit && units >= 1) {
-        int per_sm128 = 0;
-        FPT_CUDA(max_blocks_per_sm(128, &per_sm128));
-        if (per_sm128 < 1) return FPT_E_CUDA;
-        units = std::min<long long>(units, per_sm128);
-        if (!fp32 && units >= 2 && (units % 2) == 0) {          // fp64: pairs of 128 as one 256-thread block (compaction
-                                                                // works over more lanes; measured +3 %, fp32: -20 %)
-          int per_sm256 = 0;
-          FPT_CUDA(max_blocks_per_sm(256, &per_sm256));
-          if (per_sm256 >= units / 2) { block = 256; blocks = (units / 2) * sms; }
-        }
-        if (blocks == 0) { block = 128; blocks = units * sms; }
+      fn = fp32 ? persistent_kernel_f32(p->model, p->scheme, amp, ramp) : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
+      rc = ensure_dynamic_smem(fn, smem, dev);
+      if (rc != FPT_OK) return rc;
+      auto max_blocks_per_sm = [&](int blk, int* out) -> cudaError_t {
+        return cudaOccupancyMaxActiveBlocksPerMultiprocessor(out, fn, blk, smem);
+      };
+      if (explicit_geometry) {
+        // explicit geometry: block x min(blocks_per_sm, occupancy limit) per SM
+        block = cfg.block > 0 ? cfg.block : 128;
+        int per_sm = 0;
+        FPT_CUDA(max_blocks_per_sm(block, &per_sm));
+        if (per_sm < 1) return FPT_E_CUDA;
+        if (cfg.blocks_per_sm > 0) per_sm = std::min(per_sm, cfg.blocks_per_sm);
+        blocks = (long long)per_sm * sms;
       } else {
-        const long long lanes = std::min<long long>(n_traj, unit);
-        block = (int)std::min<long long>(128, std::max<long long>(32, ((lanes + sms - 1) / sms + 31) / 32 * 32));
-        blocks = (lanes + block - 1) / block;
+        // Default geometry.  Resident lanes = n_traj / R, at least one warp per SM sub-partition (128 lanes per SM) and at
+        // most what the registers allow.  R = 1 for a ramped bias (nu != 0: switching happens in a narrow window, all
+        // trajectories are about equally long, so throughput is everything); R = 5 for a constant bias (escape is a
+        // Poisson process, lengths are exponential: a launch lasts at least as long as its longest trajectory, and that
+        // one runs fastest when few warps share its SM sub-partition; the refills keep the lanes busy meanwhile).
+        const long long R = ramp ? 1 : 5;
+        // ramped: round UP, so that a job that fits resident at once runs as one wave (C4: 65536 equal-length trajectories
+        // on 4 x 128 lanes per SM, not 3 x 128 plus a straggler wave); constant bias: round down, more refills per lane
+        long long units = ramp ? (n_traj + unit - 1) / unit : n_traj / (R * unit);
+        if (n_traj >= unit && units >= 1) {
+          int per_sm128 = 0;
+          FPT_CUDA(max_blocks_per_sm(128, &per_sm128));
+          if (per_sm128 < 1) return FPT_E_CUDA;
+          units = std::min<long long>(units, per_sm128);
+          if (!fp32 && units >= 2 && (units % 2) == 0) {          // fp64: pairs of 128 as one 256-thread block (compaction
+                                                                  // works over more lanes; measured +3 %, fp32: -20 %)
+            int per_sm256 = 0;
+            FPT_CUDA(max_blocks_per_sm(256, &per_sm256));
+            if (per_sm256 >= units / 2) { block = 256; blocks = (units / 2) * sms; }
+          }
+          if (blocks == 0) { block = 128; blocks = units * sms; }
+        } else {
+          const long long lanes = std::min<long long>(n_traj, unit);
+          block = (int)std::min<long long>(128, std::max<long long>(32, ((lanes + sms - 1) / sms + 31) / 32 * 32));
+          blocks = (lanes + block - 1) / block;
+        }
       }
+      const long long needed = (n_traj + block - 1) / block;      // never more lanes than trajectories
+      if (blocks > needed) blocks = needed;
+      kernel = FPT_KERNEL_PERSISTENT;
     }
-    const long long needed = (n_traj + block - 1) / block;      // never more lanes than trajectories
-    if (blocks > needed) blocks = needed;
     if (cfg.max_blocks > 0 && blocks > cfg.max_blocks) blocks = cfg.max_blocks;
     grid = (int)blocks;
     P.schedule = cfg.schedule;
-    P.tail_helper = cfg.tail_helper;
+    P.tail_helper = cfg.tail_helper >= 0 ? 1 : 0;
     void* args[] = {(void*)&P};
     FPT_CUDA(cudaLaunchKernel(fn, dim3(grid), dim3(block), args, smem, stream));
   }
-  // keep the counters of this call for fpt_last_stats, then release the per-call workspace (stream ordered)
-  FPT_CUDA(cudaMemcpyAsync(ctx->d_last, ws, sizeof(DevStats), cudaMemcpyDeviceToDevice, stream));
-  FPT_CUDA(cudaFreeAsync(ws, stream));
-  {
-    std::lock_guard<std::mutex> lk(g_mu);
-    ctx->host = fpt_stats{};
-    ctx->host.n_traj = (uint64_t)n_traj;
-    ctx->host.n_cap = P.n_cap;
-    ctx->host.grid = grid;
-    ctx->host.block = block;
-    ctx->host.check_every = P.K;
-    ctx->last_stream = stream;
-    ctx->valid = true;
-  }
+  // this call's statistics -> the caller's block and the call's slot of the "last call" ring; then release the workspace
+  fpt_stats geo{};
+  geo.n_traj = (uint64_t)n_traj;
+  geo.n_cap = P.n_cap;
+  geo.grid = grid;
+  geo.block = block;
+  geo.check_every = P.K;
+  geo.kernel = kernel;
+  const unsigned long long ticket = ctx->next_ticket.fetch_add(1);
+  const int slot = (int)(ticket % kLastSlots);
+  fpt_export_stats_kernel<<<1, 1, 0, stream>>>(ws, geo, d_stats, ctx->d_last + slot, ctx->d_ticket + slot, ticket);
+  FPT_CUDA(cudaGetLastError());
+  t_last.ticket[dev] = ticket;
   return FPT_OK;
 }
 
@@ -502,15 +610,20 @@ extern "C" {
 
 int fpt_simulate(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
                  double* out_gamma_at_escape, int32_t* out_status, void* cuda_stream) {
-  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, false, 0, 0.0, 0.0, 0, nullptr,
-                       cuda_stream);
+  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, nullptr, nullptr, nullptr, cuda_stream);
 }
 
 int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
                       double* out_gamma_at_escape, int32_t* out_status, int32_t hist_of, double lo, double hi,
                       int32_t nbins, uint64_t* out_counts, void* cuda_stream) {
-  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, true, hist_of, lo, hi, nbins,
-                       out_counts, cuda_stream);
+  const fpt_hist h{hist_of, nbins, lo, hi, out_counts};
+  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, &h, nullptr, nullptr, cuda_stream);
+}
+
+int fpt_simulate_ex(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
+                    double* out_gamma_at_escape, int32_t* out_status, const fpt_hist* hist, const fpt_launch_opts* opts,
+                    fpt_stats* d_stats, void* cuda_stream) {
+  return simulate_impl(p, n_traj, seed, t_max, out_fpt, out_gamma_at_escape, out_status, hist, opts, d_stats, cuda_stream);
 }
 
 int fpt_histogram(const double* values, const int32_t* status, int64_t n, double lo, double hi, int32_t nbins,
@@ -537,35 +650,38 @@ int fpt_simulate_host(const fpt_params* p, int64_t n_traj, uint64_t seed, double
   if (rc != FPT_OK) return rc;
   if (n_traj == 0) return FPT_OK;
   if (!h_fpt || !h_status) return FPT_E_INVALID;
+  if (h_counts && nbins < 1) return FPT_E_INVALID;
   DeviceCtx* hctx = nullptr;
   rc = device_ctx(&hctx);
   if (rc != FPT_OK) return rc;
   cudaStream_t stream = nullptr;
   FPT_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
   const size_t n = (size_t)n_traj;
-  const size_t bytes = n * (8 + (h_gamma ? 8 : 0) + 4) + (h_counts ? (size_t)(nbins > 0 ? nbins + 2 : 0) * 8 : 0);
+  const size_t cnt_bytes = h_counts ? (size_t)(nbins + 2) * 8 : 0;
+  const size_t bytes = n * (8 + (h_gamma ? 8 : 0) + 4) + cnt_bytes;
   char* d = nullptr;
   cudaError_t e = cudaMallocFromPoolAsync((void**)&d, bytes, hctx->mem, stream);
-  if (e != cudaSuccess) { g_last_cuda = e; cudaStreamDestroy(stream); return FPT_E_CUDA; }
+  if (e != cudaSuccess) { g_last_cuda = e; (void)cudaGetLastError(); cudaStreamDestroy(stream); return FPT_E_CUDA; }
   double* d_fpt = (double*)d;
   double* d_gam = h_gamma ? d_fpt + n : nullptr;
   uint64_t* d_cnt = h_counts ? (uint64_t*)(d + n * (8 + (h_gamma ? 8 : 0))) : nullptr;
-  int32_t* d_st = (int32_t*)(d + n * (8 + (h_gamma ? 8 : 0)) + (h_counts ? (size_t)(nbins + 2) * 8 : 0));
+  int32_t* d_st = (int32_t*)(d + n * (8 + (h_gamma ? 8 : 0)) + cnt_bytes);
+  // every copy is checked; the first failure is reported after the buffer has been released and the stream drained
+  auto note = [&](cudaError_t err) { if (err != cudaSuccess && e == cudaSuccess) e = err; };
   if (h_counts) {
-    if (nbins < 1) { cudaFreeAsync(d, stream); cudaStreamDestroy(stream); return FPT_E_INVALID; }
-    cudaMemcpyAsync(d_cnt, h_counts, (size_t)(nbins + 2) * 8, cudaMemcpyHostToDevice, stream);
-    rc = fpt_simulate_hist(p, n_traj, seed, t_max, d_fpt, d_gam, d_st, hist_of, lo, hi, nbins, d_cnt, stream);
+    note(cudaMemcpyAsync(d_cnt, h_counts, cnt_bytes, cudaMemcpyHostToDevice, stream));
+    if (e == cudaSuccess) rc = fpt_simulate_hist(p, n_traj, seed, t_max, d_fpt, d_gam, d_st, hist_of, lo, hi, nbins, d_cnt, stream);
   } else {
     rc = fpt_simulate(p, n_traj, seed, t_max, d_fpt, d_gam, d_st, stream);
   }
-  if (rc == FPT_OK) {
-    cudaMemcpyAsync(h_fpt, d_fpt, n * 8, cudaMemcpyDeviceToHost, stream);
-    if (h_gamma) cudaMemcpyAsync(h_gamma, d_gam, n * 8, cudaMemcpyDeviceToHost, stream);
-    cudaMemcpyAsync(h_status, d_st, n * 4, cudaMemcpyDeviceToHost, stream);
-    if (h_counts) cudaMemcpyAsync(h_counts, d_cnt, (size_t)(nbins + 2) * 8, cudaMemcpyDeviceToHost, stream);
+  if (rc == FPT_OK && e == cudaSuccess) {
+    note(cudaMemcpyAsync(h_fpt, d_fpt, n * 8, cudaMemcpyDeviceToHost, stream));
+    if (h_gamma) note(cudaMemcpyAsync(h_gamma, d_gam, n * 8, cudaMemcpyDeviceToHost, stream));
+    note(cudaMemcpyAsync(h_status, d_st, n * 4, cudaMemcpyDeviceToHost, stream));
+    if (h_counts) note(cudaMemcpyAsync(h_counts, d_cnt, cnt_bytes, cudaMemcpyDeviceToHost, stream));
   }
-  cudaFreeAsync(d, stream);
-  e = cudaStreamSynchronize(stream);
+  note(cudaFreeAsync(d, stream));
+  note(cudaStreamSynchronize(stream));
   cudaStreamDestroy(stream);
   if (rc == FPT_OK && e != cudaSuccess) { g_last_cuda = e; (void)cudaGetLastError(); return FPT_E_CUDA; }
   return rc;
@@ -583,78 +699,91 @@ int fpt_simulate_sweep(const fpt_params* sets, int32_t n_sets, int64_t n_per_set
   DeviceCtx* ctx = nullptr;
   int rc = device_ctx(&ctx);
   if (rc != FPT_OK) return rc;
-  {
-    std::lock_guard<std::mutex> lk(g_mu);
-    if (!ctx->pool_ready) {
-      for (int i = 0; i < kSweepStreams; ++i) {
-        FPT_CUDA(cudaStreamCreateWithFlags(&ctx->pool[i], cudaStreamNonBlocking));
-        FPT_CUDA(cudaEventCreateWithFlags(&ctx->pool_done[i], cudaEventDisableTiming));
-      }
-      FPT_CUDA(cudaEventCreateWithFlags(&ctx->fork, cudaEventDisableTiming));
-      ctx->pool_ready = true;
-    }
+  // one sweep at a time per device on the stream pool (the launches of two sweeps would interleave on it otherwise); the
+  // section only enqueues, so the lock is held for microseconds per set
+  std::lock_guard<std::mutex> lk(ctx->mu);
+  if (!ctx->pool_ready) {
+    for (int i = 0; i < kSweepStreams; ++i) FPT_CUDA(cudaStreamCreateWithFlags(&ctx->pool[i], cudaStreamNonBlocking));
+    ctx->pool_ready = true;
   }
   cudaStream_t caller = (cudaStream_t)cuda_stream;
   const int used = n_sets < kSweepStreams ? n_sets : kSweepStreams;
+  // per-call events: recorded, waited on and destroyed here (the runtime defers the destruction until they complete)
+  cudaEvent_t fork = nullptr, done[kSweepStreams] = {};
+  cudaError_t e = cudaEventCreateWithFlags(&fork, cudaEventDisableTiming);
+  for (int i = 0; i < used && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&done[i], cudaEventDisableTiming);
+  int forked = 0;
   // fork: the pool streams start after everything already queued on the caller's stream
-  FPT_CUDA(cudaEventRecord(ctx->fork, caller));
-  for (int i = 0; i < used; ++i) FPT_CUDA(cudaStreamWaitEvent(ctx->pool[i], ctx->fork, 0));
-  for (int32_t i = 0; i < n_sets && rc == FPT_OK; ++i) {
+  if (e == cudaSuccess) e = cudaEventRecord(fork, caller);
+  for (int i = 0; i < used && e == cudaSuccess; ++i) {
+    e = cudaStreamWaitEvent(ctx->pool[i], fork, 0);
+    if (e == cudaSuccess) forked = i + 1;
+  }
+  for (int32_t i = 0; i < n_sets && rc == FPT_OK && e == cudaSuccess; ++i) {
     const size_t off = (size_t)i * (size_t)n_per_set;
     rc = simulate_impl(&sets[i], n_per_set, seed, t_max[i], out_fpt + off, out_gamma_at_escape ? out_gamma_at_escape + off : nullptr,
-                       out_status + off, false, 0, 0.0, 0.0, 0, nullptr, ctx->pool[i % kSweepStreams]);
+                       out_status + off, nullptr, nullptr, nullptr, ctx->pool[i % kSweepStreams]);
   }
-  // join: the caller's stream continues when every set is done (also after a failed launch, so nothing dangles)
-  for (int i = 0; i < used; ++i) {
-    FPT_CUDA(cudaEventRecord(ctx->pool_done[i], ctx->pool[i]));
-    FPT_CUDA(cudaStreamWaitEvent(caller, ctx->pool_done[i], 0));
+  // join, ALWAYS (also after a failed launch): the caller's stream continues when every forked pool stream is done
+  for (int i = 0; i < forked; ++i) {
+    cudaError_t e2 = cudaEventRecord(done[i], ctx->pool[i]);
+    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(caller, done[i], 0);
+    if (e2 != cudaSuccess && e == cudaSuccess) e = e2;
   }
+  if (fork) cudaEventDestroy(fork);
+  for (int i = 0; i < used; ++i)
+    if (done[i]) cudaEventDestroy(done[i]);
+  if (rc == FPT_OK && e != cudaSuccess) { g_last_cuda = e; (void)cudaGetLastError(); return FPT_E_CUDA; }
   return rc;
 }
 
 int fpt_set_launch(int32_t block, int32_t blocks_per_sm, int32_t max_blocks) {
-  if (block != 0 && (block < 32 || block > 256 || (block % 32) != 0)) return FPT_E_INVALID;
-  if (blocks_per_sm < 0 || blocks_per_sm > 64 || max_blocks < 0) return FPT_E_INVALID;
-  std::lock_guard<std::mutex> lk(g_mu);
-  g_cfg.block = block;
-  g_cfg.blocks_per_sm = blocks_per_sm;
-  g_cfg.max_blocks = max_blocks;
+  fpt_launch_opts o = t_opts;
+  o.block = block;
+  o.blocks_per_sm = blocks_per_sm;
+  o.max_blocks = max_blocks;
+  if (validate_opts(&o) != FPT_OK) return FPT_E_INVALID;
+  t_opts = o;
   return FPT_OK;
 }
 
 int fpt_set_schedule(int32_t schedule) {
   if (schedule != FPT_SCHEDULE_DYNAMIC && schedule != FPT_SCHEDULE_STATIC) return FPT_E_INVALID;
-  std::lock_guard<std::mutex> lk(g_mu);
-  g_cfg.schedule = schedule;
+  t_opts.schedule = schedule;
   return FPT_OK;
 }
 
 int fpt_set_tail_helper(int32_t on) {
   if (on != 0 && on != 1) return FPT_E_INVALID;
-  std::lock_guard<std::mutex> lk(g_mu);
-  g_cfg.tail_helper = on;
+  t_opts.tail_helper = on ? 1 : -1;
+  return FPT_OK;
+}
+
+int fpt_set_specialise(int32_t specialise, int32_t consumers, int32_t producers) {
+  fpt_launch_opts o = t_opts;
+  o.specialise = specialise;
+  o.consumers = consumers;
+  o.producers = producers;
+  if (validate_opts(&o) != FPT_OK) return FPT_E_INVALID;
+  t_opts = o;
   return FPT_OK;
 }
 
 int fpt_last_stats(fpt_stats* out) {
   if (!out) return FPT_E_INVALID;
   DeviceCtx* ctx = nullptr;
-  int rc = device_ctx(&ctx);
+  int dev = 0;
+  int rc = device_ctx(&ctx, &dev);
   if (rc != FPT_OK) return rc;
+  std::memset(out, 0, sizeof(*out));
+  const unsigned long long ticket = t_last.ticket[dev];
+  if (ticket == 0) return FPT_OK;                              // this thread has made no call on this device
   FPT_CUDA(cudaDeviceSynchronize());
-  DevStats h;
-  FPT_CUDA(cudaMemcpy(&h, ctx->d_last, sizeof(h), cudaMemcpyDeviceToHost));
-  std::lock_guard<std::mutex> lk(g_mu);
-  if (!ctx->valid) { std::memset(out, 0, sizeof(*out)); return FPT_OK; }
-  *out = ctx->host;
-  out->n_escaped = h.n_escaped;
-  out->n_censored = h.n_censored;
-  out->n_nan = h.n_nan;
-  out->useful_steps = h.useful_steps;
-  out->issued_lane_steps = h.issued_lane_steps;
-  out->refill_atomics = h.refill_atomics;
-  out->migrations = h.migrations;
-  out->helper_lane_steps = h.helper_lane_steps;
+  const int slot = (int)(ticket % kLastSlots);
+  unsigned long long owner = 0;
+  FPT_CUDA(cudaMemcpy(&owner, ctx->d_ticket + slot, sizeof(owner), cudaMemcpyDeviceToHost));
+  if (owner != ticket) return FPT_OK;                          // kLastSlots later calls have recycled the slot: zeros
+  FPT_CUDA(cudaMemcpy(out, ctx->d_last + slot, sizeof(*out), cudaMemcpyDeviceToHost));
   return FPT_OK;
 }
 
@@ -670,7 +799,7 @@ const char* fpt_strerror(int code) {
   }
 }
 
-int fpt_version(void) { return 102; }
+int fpt_version(void) { return 200; }
 
 // ---- test hooks
 int fpt_dbg_philox(uint64_t seed, uint64_t id0, int64_t n_ids, uint64_t block, uint32_t* out, void* s) {
@@ -730,6 +859,10 @@ int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t bl
   FPT_CUDA(cudaGetLastError());
   return FPT_OK;
 }
+int fpt_dbg_set_helper_seq0(uint64_t seq0) {
+  t_dbg_seq0 = seq0;
+  return FPT_OK;
+}
 int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len, double* trace_phi,
                   double* trace_v, int32_t* out_status, uint64_t* out_k_end, void* s) {
   int rc = validate(p, 0, t_max);
@@ -738,7 +871,10 @@ int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max,
   KParams P;
   derive(*p, t_max, seed, P);
   TraceArgs T{id, trace_len, trace_phi, trace_v, out_status, (unsigned long long*)out_k_end};
-  const void* fn = p->precision == FPT_PREC_FP32 ? trace_kernel_f32(p->model, p->scheme) : trace_kernel_f64(p->model, p->scheme);
+  // the same State specialisation as the production launch of these parameters (R15 shortcuts included)
+  const bool amp = p->amp != 0.0, ramp = p->nu != 0.0;
+  const void* fn = p->precision == FPT_PREC_FP32 ? trace_kernel_f32(p->model, p->scheme, amp, ramp)
+                                                 : trace_kernel_f64(p->model, p->scheme, amp, ramp);
   void* args[] = {(void*)&P, (void*)&T};
   FPT_CUDA(cudaLaunchKernel(fn, dim3(1), dim3(32), args, 0, (cudaStream_t)s));
   return FPT_OK;

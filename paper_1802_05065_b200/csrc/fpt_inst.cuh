@@ -1,7 +1,8 @@
-// fpt_inst.cuh -- kernel-pointer tables.  The 2 x 16 instantiations of the persistent kernel are split over two
-// translation units (fpt_inst64.cu, fpt_inst32.cu) so that they compile in parallel; the API unit only sees these
+// fpt_inst.cuh -- kernel-pointer tables.  The 2 x (16 + 8) instantiations of the two integrator kernels are split over
+// two translation units (fpt_inst64.cu, fpt_inst32.cu) so that they compile in parallel; the API unit only sees these
 // lookups.
 #pragma once
+#include <cstddef>
 #include <cuda_runtime.h>
 
 namespace fpt {
@@ -9,8 +10,11 @@ namespace fpt {
 // persistent integrator for (model, scheme, amp != 0, nu != 0)
 const void* persistent_kernel_f64(int model, int scheme, bool amp, bool ramp);
 const void* persistent_kernel_f32(int model, int scheme, bool amp, bool ramp);
-// single-trajectory tracer (test hook), general amp / ramp code path
-const void* trace_kernel_f64(int model, int scheme);
-const void* trace_kernel_f32(int model, int scheme);
+// warp-specialised integrator (drifts with a sine only: amp != 0); *channel_bytes = dynamic shared memory per consumer
+const void* specialised_kernel_f64(int model, int scheme, bool ramp, size_t* channel_bytes);
+const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* channel_bytes);
+// single-trajectory tracer (test hook): the same State specialisation the production launch picks
+const void* trace_kernel_f64(int model, int scheme, bool amp, bool ramp);
+const void* trace_kernel_f32(int model, int scheme, bool amp, bool ramp);
 
 }  // namespace fpt

@@ -1,32 +1,12 @@
-// fpt_inst64.cu -- instantiations of the persistent integrator and the tracer for the fp64 state (see fpt_inst.cuh).
-#include "fpt_inst.cuh"
-#include "fpt_integrator.cuh"
+// fpt_inst64.cu -- instantiations of the integrator kernels and the tracer for the fp64 state (see fpt_inst.cuh).
+#include "fpt_inst_impl.cuh"
 
 namespace fpt {
 
-namespace {
-template <int M, int S, bool A, bool R>
-const void* pk() {
-  return (const void*)&fpt_persistent_kernel<State64<M, S, A, R>>;
+const void* persistent_kernel_f64(int model, int scheme, bool amp, bool ramp) { return Inst<State64>::persistent(model, scheme, amp, ramp); }
+const void* specialised_kernel_f64(int model, int scheme, bool ramp, size_t* channel_bytes) {
+  return Inst<State64>::specialised(model, scheme, ramp, channel_bytes);
 }
-template <int M, int S>
-const void* pick_ar(bool a, bool r) {
-  if (a) return r ? pk<M, S, true, true>() : pk<M, S, true, false>();
-  return r ? pk<M, S, false, true>() : pk<M, S, false, false>();
-}
-}  // namespace
-
-const void* persistent_kernel_f64(int model, int scheme, bool amp, bool ramp) {
-  if (model == 0) return scheme == 0 ? pick_ar<0, 0>(amp, ramp) : pick_ar<0, 1>(amp, ramp);
-  return scheme == 0 ? pick_ar<1, 0>(amp, ramp) : pick_ar<1, 1>(amp, ramp);
-}
-
-const void* trace_kernel_f64(int model, int scheme) {
-  if (model == 0)
-    return scheme == 0 ? (const void*)&fpt_trace_kernel<State64<0, 0, true, true>>
-                       : (const void*)&fpt_trace_kernel<State64<0, 1, true, true>>;
-  return scheme == 0 ? (const void*)&fpt_trace_kernel<State64<1, 0, true, true>>
-                     : (const void*)&fpt_trace_kernel<State64<1, 1, true, true>>;
-}
+const void* trace_kernel_f64(int model, int scheme, bool amp, bool ramp) { return Inst<State64>::trace(model, scheme, amp, ramp); }
 
 }  // namespace fpt

@@ -20,10 +20,14 @@ def lib():
 
 
 def test_exports_every_declared_symbol(lib):
-    header = (ROOT / "include" / "fpt.h").read_text()
-    code = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
-    declared = set(re.findall(r"\b(fpt_[a-z0-9_]+)\s*\(", code))
-    assert len(declared) >= 15
+    declared = set()
+    for name in ("fpt.h", "fpt_dbg.h"):               # product API + test hooks / microbenchmarks
+        header = (ROOT / "include" / name).read_text()
+        code = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+        declared |= set(re.findall(r"\b(fpt_[a-z0-9_]+)\s*\(", code))
+    assert len(declared) >= 25
+    product = re.sub(r"/\*.*?\*/", "", (ROOT / "include" / "fpt.h").read_text(), flags=re.S)
+    assert "fpt_dbg_" not in product and "_peak" not in product      # hooks live in fpt_dbg.h only
     for name in declared:
         assert hasattr(lib, name), name
     assert declared == set(binding.EXPORTS)          # the binding covers the whole header, and nothing else
@@ -33,8 +37,10 @@ def test_struct_layouts(lib):
     assert C.sizeof(fpt.FptParams) == 96              # 4 x int32, 9 x double, 1 x uint64, no padding
     assert fpt.FptParams.first_id.offset == 88
     assert C.sizeof(fpt.FptStats) == 96
-    assert fpt.FptStats.migrations.offset == 80
-    assert fpt.version() >= 100
+    assert fpt.FptStats.migrations.offset == 80 and fpt.FptStats.kernel.offset == 76
+    assert C.sizeof(fpt.FptLaunchOpts) == 32 and fpt.FptLaunchOpts.producers.offset == 28
+    assert C.sizeof(fpt.FptHist) == 32 and fpt.FptHist.out_counts.offset == 24
+    assert fpt.version() >= 200
 
 
 def test_strerror(lib):
@@ -77,6 +83,22 @@ def test_invalid_call_arguments(lib):
     assert lib.fpt_histogram(None, None, 5, 0.0, 1.0, 4, C.c_void_p(8), None) == -1
     assert lib.fpt_histogram(C.c_void_p(8), None, 5, 1.0, 0.0, 4, C.c_void_p(8), None) == -1
     assert lib.fpt_histogram(C.c_void_p(8), None, 0, 0.0, 1.0, 4, C.c_void_p(8), None) == 0
+    # fpt_simulate_ex: bad launch options / histogram request are rejected before any CUDA work
+    ex = lambda opts=None, hist=None: lib.fpt_simulate_ex(C.byref(p), 10, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8),
+                                                          C.byref(hist) if hist else None, C.byref(opts) if opts else None, None, None)
+    assert ex(fpt.FptLaunchOpts(block=48)) == -1
+    assert ex(fpt.FptLaunchOpts(block=512)) == -1
+    assert ex(fpt.FptLaunchOpts(schedule=2)) == -1
+    assert ex(fpt.FptLaunchOpts(tail_helper=2)) == -1
+    assert ex(fpt.FptLaunchOpts(specialise=-2)) == -1
+    assert ex(fpt.FptLaunchOpts(consumers=5)) == -1
+    assert ex(fpt.FptLaunchOpts(producers=4)) == -1
+    assert ex(fpt.FptLaunchOpts(max_blocks=-1)) == -1
+    assert ex(None, fpt.FptHist(0, 0, 0.0, 1.0, 8)) == -1
+    assert ex(None, fpt.FptHist(2, 10, 0.0, 1.0, 8)) == -1
+    assert ex(None, fpt.FptHist(0, 10, 0.0, 1.0, None)) == -1
+    assert lib.fpt_simulate_ex(C.byref(p), 0, 1, 1.0, None, None, None, None, None, None, None) == 0
+    assert lib.fpt_set_specialise(2, 0, 0) == -1 and lib.fpt_set_specialise(0, 0, 0) == 0
     assert lib.fpt_set_launch(48, 0, 0) == -1
     assert lib.fpt_set_launch(512, 0, 0) == -1
     assert lib.fpt_set_launch(128, 2, 0) == 0

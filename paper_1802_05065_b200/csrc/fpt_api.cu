@@ -295,17 +295,21 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     size_t smem = hist_bytes;
     long long blocks = 0;
     if (spec) {
-      size_t chan = 0;
-      fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &chan) : specialised_kernel_f64(p->model, p->scheme, ramp, &chan);
+      size_t fixed = 0, chan = 0;
+      fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &fixed, &chan)
+                : specialised_kernel_f64(p->model, p->scheme, ramp, &fixed, &chan);
       int NC = cfg.consumers > 0 ? cfg.consumers : 4;
-      const int NP = cfg.producers > 0 ? cfg.producers : 2;
+      const int NP = cfg.producers > 0 ? cfg.producers : 1;
       // few trajectories: fewer consumers per block, so that every SM gets some
       while (cfg.consumers == 0 && NC > 1 && (long long)(NC - 1) * 32 * sms >= n_traj) --NC;
       P.spec_consumers = NC;
       P.spec_producers = NP;
+      // a consumer must not share its SM sub-partition with a producer (fpt_specialised.cuh): with one producer each and
+      // more than two consumers, even warps consume and odd warps produce
+      P.spec_layout = (NP == 1 && NC > 2) ? 1 : 0;
       P.K = fp32 ? kSpecChunk32 : kSpecChunk64;                   // one poll per hand-over chunk
       block = 32 * NC * (1 + NP);
-      smem = (size_t)NC * chan + hist_bytes;
+      smem = fixed + (size_t)NC * chan + hist_bytes;
       rc = ensure_dynamic_smem(fn, smem, dev);
       if (rc != FPT_OK) return rc;
       int per_sm = 0;
@@ -719,10 +723,14 @@ int fpt_simulate_sweep(const fpt_params* sets, int32_t n_sets, int64_t n_per_set
     e = cudaStreamWaitEvent(ctx->pool[i], fork, 0);
     if (e == cudaSuccess) forked = i + 1;
   }
+  // the sets run side by side: when together they fill the GPU no warp runs alone, and the persistent kernel (every warp
+  // self-sufficient, little shared memory, several blocks per SM) is the one to use for each of them
+  fpt_launch_opts opts = t_opts;
+  if (opts.specialise == 0 && (long long)n_sets * n_per_set >= 256LL * ctx->sm_count) opts.specialise = -1;
   for (int32_t i = 0; i < n_sets && rc == FPT_OK && e == cudaSuccess; ++i) {
     const size_t off = (size_t)i * (size_t)n_per_set;
     rc = simulate_impl(&sets[i], n_per_set, seed, t_max[i], out_fpt + off, out_gamma_at_escape ? out_gamma_at_escape + off : nullptr,
-                       out_status + off, nullptr, nullptr, nullptr, ctx->pool[i % kSweepStreams]);
+                       out_status + off, nullptr, &opts, nullptr, ctx->pool[i % kSweepStreams]);
   }
   // join, ALWAYS (also after a failed launch): the caller's stream continues when every forked pool stream is done
   for (int i = 0; i < forked; ++i) {

@@ -10,9 +10,10 @@ namespace fpt {
 // persistent integrator for (model, scheme, amp != 0, nu != 0)
 const void* persistent_kernel_f64(int model, int scheme, bool amp, bool ramp);
 const void* persistent_kernel_f32(int model, int scheme, bool amp, bool ramp);
-// warp-specialised integrator (drifts with a sine only: amp != 0); *channel_bytes = dynamic shared memory per consumer
-const void* specialised_kernel_f64(int model, int scheme, bool ramp, size_t* channel_bytes);
-const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* channel_bytes);
+// warp-specialised integrator (drifts with a sine only: amp != 0); dynamic shared memory = *fixed_bytes + consumers x
+// *channel_bytes (+ the histogram bins)
+const void* specialised_kernel_f64(int model, int scheme, bool ramp, size_t* fixed_bytes, size_t* channel_bytes);
+const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* fixed_bytes, size_t* channel_bytes);
 // single-trajectory tracer (test hook): the same State specialisation the production launch picks
 const void* trace_kernel_f64(int model, int scheme, bool amp, bool ramp);
 const void* trace_kernel_f32(int model, int scheme, bool amp, bool ramp);

@@ -4,8 +4,8 @@
 namespace fpt {
 
 const void* persistent_kernel_f32(int model, int scheme, bool amp, bool ramp) { return Inst<State32>::persistent(model, scheme, amp, ramp); }
-const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* channel_bytes) {
-  return Inst<State32>::specialised(model, scheme, ramp, channel_bytes);
+const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* fixed_bytes, size_t* channel_bytes) {
+  return Inst<State32>::specialised(model, scheme, ramp, fixed_bytes, channel_bytes);
 }
 const void* trace_kernel_f32(int model, int scheme, bool amp, bool ramp) { return Inst<State32>::trace(model, scheme, amp, ramp); }
 

@@ -34,7 +34,8 @@ struct Inst {
     if (model == 0) return scheme == 0 ? pick_t<0, 0>(a, r) : pick_t<0, 1>(a, r);
     return scheme == 0 ? pick_t<1, 0>(a, r) : pick_t<1, 1>(a, r);
   }
-  static const void* specialised(int model, int scheme, bool r, size_t* channel_bytes) {
+  static const void* specialised(int model, int scheme, bool r, size_t* fixed_bytes, size_t* channel_bytes) {
+    *fixed_bytes = spec_pool_bytes();
     *channel_bytes = spec_channel_bytes<St<0, 0, true, true>>();      // depends on the precision only
     if (model == 0) {
       if (scheme == 0) return r ? sk<0, 0, true>() : sk<0, 0, false>();

@@ -45,7 +45,10 @@ def same_bits(a, b):
     return a.shape == b.shape and np.array_equal(na, nb) and np.array_equal(a[~na].view(view), b[~nb].view(view))
 
 
-def run_gpu(w, n=None, first_id=0, check_every=0, hist=False):
+def run_gpu(w, n=None, first_id=0, check_every=0, hist=False, both=True):
+    """One call through the plain API (library defaults, or whatever fpt.set_* the test has made).  For drifts with a sine
+    the same job is then repeated through fpt_simulate_ex on BOTH integrator kernels (persistent, warp-specialised) and
+    must give the same bits: every parity test below therefore covers both."""
     kw = dict(w["params"], first_id=first_id, check_every=check_every)
     p = fpt.make_params(**kw)
     n = w["n_traj"] if n is None else n
@@ -53,10 +56,27 @@ def run_gpu(w, n=None, first_id=0, check_every=0, hist=False):
         of, lo, hi, nb = w["hist"]
         f, g, s, c = fpt.simulate_hist(p, n, w["seed"], w["t_max"], lo, hi, nb, hist_of=of)
         torch.cuda.synchronize()
-        return _np(f), _np(g), _np(s), _np(c).astype(np.uint64)
-    f, g, s = fpt.simulate(p, n, w["seed"], w["t_max"])
-    torch.cuda.synchronize()
-    return _np(f), _np(g), _np(s)
+        out = _np(f), _np(g), _np(s), _np(c).astype(np.uint64)
+    else:
+        f, g, s = fpt.simulate(p, n, w["seed"], w["t_max"])
+        torch.cuda.synchronize()
+        out = _np(f), _np(g), _np(s)
+    run_gpu.stats = fpt.last_stats()                    # statistics of the primary call
+    if both and n > 0 and w["params"].get("amp", 1.0) != 0.0:
+        decided_at_once = run_gpu.stats["kernel"] == 0
+        for spec in (True, False):
+            st = fpt.alloc_stats()
+            h = None
+            if hist:
+                cnt = torch.zeros(nb + 2, dtype=torch.int64, device="cuda")
+                h = (of, lo, hi, nb, cnt)
+            f2, g2, s2 = fpt.simulate_ex(p, n, w["seed"], w["t_max"], hist=h, opts=fpt.launch_opts(specialise=spec), stats=st)
+            torch.cuda.synchronize()
+            o2 = (_np(f2), _np(g2), _np(s2)) + ((_np(cnt).astype(np.uint64),) if hist else ())
+            assert all(same_bits(a, b) if a.dtype.kind == "f" else np.array_equal(a, b) for a, b in zip(o2, out)), spec
+            if not decided_at_once:
+                assert fpt.read_stats(st)["kernel"] == (2 if spec else 1)
+    return out
 
 
 def run_oracle(w, n, first_id=0):
@@ -207,7 +227,7 @@ def test_config2_subset_with_refill():
     fpt.set_launch(64, 1, 8)                          # 512 lanes for 5003 trajectories: every lane refills ~10 times
     try:
         gpu = run_gpu(w, n)
-        stats = fpt.last_stats()
+        stats = run_gpu.stats
     finally:
         fpt.set_launch(0, 0, 0)
     ora = run_oracle(w, n)
@@ -254,7 +274,7 @@ def test_config5_family_imbalanced():
     assert_parity(gpu, ora, w["params"]["dt"], REL_FP64)
     ncens = int(np.sum(ora["status"] == 1))
     assert 0 < ncens < n // 2
-    assert fpt.last_stats()["n_censored"] == ncens
+    assert run_gpu.stats["n_censored"] == ncens
     w2 = fpt.workload("c5", temperature=0.2)
     f, g, s = run_gpu(w2, 4)
     assert [int(round(t / 5e-3)) for t in f] == [5625, 11381, 16955, 21480]
@@ -319,7 +339,7 @@ def test_drain_compaction_parks_and_adopts_without_changing_results():
         fpt.set_launch(256, 1, n // 256)                 # every trajectory resident at once: the whole run is a drain
         try:
             gpu = run_gpu(w, n, check_every=8)
-            st = fpt.last_stats()
+            st = run_gpu.stats
         finally:
             fpt.set_launch(0, 0, 0)
         ora = run_oracle(w, n)
@@ -349,7 +369,7 @@ def test_tail_helper_serves_the_last_warp_without_changing_results():
             fpt.set_launch(128, 1, n // 128)            # every trajectory resident: blocks of 4 warps drain down to one
             try:
                 gpu = run_gpu(w, n, check_every=K)
-                st = fpt.last_stats()
+                st = run_gpu.stats
             finally:
                 fpt.set_launch(0, 0, 0)
                 fpt.set_tail_helper(True)
@@ -360,14 +380,10 @@ def test_tail_helper_serves_the_last_warp_without_changing_results():
         assert all(np.array_equal(a, b) for a, b in zip(*outs))
     # a poll interval that is not a multiple of the hand-over chunk, or blocks of fewer than three warps: the helper stays off
     w = fpt.workload("c2", t_max=100.0)
-    run_gpu(w, 512, check_every=48)
-    assert fpt.last_stats()["helper_lane_steps"] == 0
-    fpt.set_launch(64, 1, 8)
-    try:
-        run_gpu(w, 512, check_every=64)
-        assert fpt.last_stats()["helper_lane_steps"] == 0
-    finally:
-        fpt.set_launch(0, 0, 0)
+    for opts, K in [(fpt.launch_opts(block=128, blocks_per_sm=1, max_blocks=4), 48), (fpt.launch_opts(block=64, blocks_per_sm=1, max_blocks=8), 64)]:
+        st = fpt.alloc_stats()
+        fpt.simulate_ex(fpt.make_params(**dict(w["params"], check_every=K)), 512, w["seed"], w["t_max"], opts=opts, stats=st)
+        assert fpt.read_stats(st)["helper_lane_steps"] == 0 and fpt.read_stats(st)["kernel"] == 1
 
 
 def test_concurrent_streams_and_host_threads():
@@ -478,7 +494,7 @@ def test_edge_cases():
         ora = run_oracle(ww, 64)
         assert oracle.n_cap(oracle.make_params(**ww["params"]), ww["t_max"]) == n_cap
         assert_parity(gpu, ora, 0.01, REL_FP64)
-        assert fpt.last_stats()["n_cap"] == n_cap
+        assert run_gpu.stats["n_cap"] == n_cap
     # initial state already beyond the threshold: escaped at k = 0
     ww = fpt.workload("c2", threshold=1.0)
     gpu = run_gpu(ww, 100)
@@ -503,7 +519,7 @@ def test_edge_cases():
         bad = ora["status"] == 2
         assert np.all(np.isnan(gpu[0][bad])) and np.all(np.isnan(gpu[1][bad]))
         assert np.array_equal(gpu[0][~bad], ora["fpt"][~bad])
-        assert fpt.last_stats()["n_nan"] == int(bad.sum())
+        assert run_gpu.stats["n_nan"] == int(bad.sum())
 
 
 def test_host_buffer_entry_point_matches_device_path():
@@ -531,7 +547,7 @@ def test_config2_full_size_sampled():
     w = fpt.workload("c2")
     n = w["n_traj"]
     f, g, s = run_gpu(w)
-    stats = fpt.last_stats()
+    stats = run_gpu.stats
     assert stats["n_traj"] == n and stats["n_escaped"] + stats["n_censored"] + stats["n_nan"] == n
     k = np.rint(f / 0.01).astype(np.int64)
     assert np.all(s == 0) and stats["useful_steps"] == int(k.sum())

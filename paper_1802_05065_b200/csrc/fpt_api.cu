@@ -32,9 +32,13 @@ thread_local cudaError_t g_last_cuda = cudaSuccess;
   } while (0)
 
 constexpr int kMaxDevices = 64;
-// default poll interval in steps: measured on B200, a poll costs about as much as 1.3 steps (the software pipeline of the
-// step loop drains and refills around it), so 64 (fp64) / 32 (fp32) steps keep it near 2 %; a finished lane idles K/2 steps
-constexpr int kDefaultK64 = 64, kDefaultK32 = 32;
+// default poll interval in steps: measured on B200, a poll costs about as much as 1.3 steps in fp64 and 3 in fp32 (the
+// software pipeline of the step loop drains and refills around it), and a finished lane idles K/2 steps on average, so
+// the best K grows with the square root of the trajectory length.  The cap is all the host knows about that length:
+// fp64 64, and 128 from caps of 2^21 steps (configs 3 and 5: +0.5 %, +1 %; config 2, cap 10^6 and mean 5700: -0.4 %);
+// fp32 64, and 128 from caps of 2^16 steps (config 4 twin: +3.8 % over 32; 256 is no better)
+constexpr int kDefaultK = 64, kDefaultKLong = 128;
+constexpr unsigned long long kLongCap64 = 1ull << 21, kLongCap32 = 1ull << 16;
 // specialised kernel (fpt_specialised.cuh): hand-over chunk = its poll interval; limits of fpt_launch_opts
 constexpr int kSpecChunk64 = 64, kSpecChunk32 = 32;
 constexpr int kSpecMaxConsumersHost = 4, kSpecMaxProducersHost = 3;
@@ -160,7 +164,8 @@ void derive(const fpt_params& p, double t_max, uint64_t seed, KParams& P) {
   P.first_id = p.first_id;
   P.n_cap = (unsigned long long)std::nearbyint(t_max / p.dt);
   const int macro = p.precision == FPT_PREC_FP32 ? 4 : 2;
-  int K = p.check_every > 0 ? p.check_every : (p.precision == FPT_PREC_FP32 ? kDefaultK32 : kDefaultK64);
+  const unsigned long long long_cap = p.precision == FPT_PREC_FP32 ? kLongCap32 : kLongCap64;
+  int K = p.check_every > 0 ? p.check_every : (P.n_cap >= long_cap ? kDefaultKLong : kDefaultK);
   K = ((K + macro - 1) / macro) * macro;
   P.K = K;
   P.hist_of = -1;

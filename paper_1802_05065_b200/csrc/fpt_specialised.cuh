@@ -239,30 +239,27 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
       }
       __threadfence_block();
       // ---- kChunk steps (S3..S6), sticky per-step escape capture as in the persistent kernel
-      int n_alive = 0;
-      int cap_hi = 0;
-      bool alive = true;
+      EscapeCapture cap;
+      cap.reset();
       const real* zb = zbuf + (size_t)(cseq & 1ull) * (kChunk * 32) + lane;
 #pragma unroll 8
       for (int s = 0; s < kChunk; ++s) {
         st.step(P, zb[s * 32]);
-        if (alive) cap_hi = st.phi_hi();
-        alive = alive && !st.crossed(P);
-        if (alive) ++n_alive;
+        cap.observe(st, P);
       }
       ++cseq;
       ++s_chunks;
       // ---- classify (S6 / cap) and write results by trajectory id
       const unsigned long long rem = P.n_cap - kbase;
-      const bool fin = active && (!alive || rem <= (unsigned long long)kChunk);
+      const bool fin = active && (!cap.alive || rem <= (unsigned long long)kChunk);
       if (__any_sync(0xffffffffu, fin)) {
         if (fin) {
           int status = kStatusCensored;
           unsigned long long k_end = P.n_cap;
-          const int koff = n_alive + 1;                       // step offset (1..kChunk) of the first crossing in this chunk
-          if (!alive && (unsigned long long)koff <= rem) {
+          const int koff = cap.k_fail();                       // step offset (1..kChunk) of the first crossing in this chunk
+          if (!cap.alive && (unsigned long long)koff <= rem) {
             k_end = kbase + (unsigned long long)koff;
-            status = st.is_nan_hi(cap_hi) ? kStatusNan : kStatusEscaped;
+            status = st.is_nan_hi(cap.cap_hi) ? kStatusNan : kStatusEscaped;
           }
           const double kf = __ull2double_rn(k_end);           // exact: k_end < 2^53
           double fptv = __dmul_rn(kf, P.dt);

@@ -31,10 +31,59 @@ if ROOT not in sys.path:
 METRIC = "trajectory-steps/s"
 UNIT = "steps/s"
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE persistent-kernel launch of the bench workload (C2, 10^5 trajectories),
-# from the `ncu --set full` capture summarised in profiles/r01e_README.md: 53 248 B read, 0 B written (the 2 MB of outputs
-# are still in the 126 MB L2 when the kernel ends).  Only valid for that workload; None for any other.
-NCU_DRAM_BYTES_PER_LAUNCH = 53248
+PROFILES = os.path.join(ROOT, "profiles")
+
+
+def kernel_source_sha() -> str:
+    """sha256 over the CUDA sources the kernels are built from: ties a stored measurement to the code it was taken on."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1802_05065_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload: str, n_traj: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE integrator launch of this workload, from the `ncu --set full`
+    capture recorded in profiles/ncu_traffic.json -- or None when there is no capture of this workload, or the kernel
+    sources have changed since it was taken (the record carries their hash)."""
+    try:
+        rec = json.load(open(os.path.join(PROFILES, "ncu_traffic.json")))
+    except (OSError, ValueError):
+        return None, "no profiles/ncu_traffic.json"
+    e = rec.get("captures", {}).get(f"{workload}@{n_traj}")
+    if e is None:
+        return None, "no capture of this workload"
+    if e.get("kernel_source_sha") != kernel_source_sha():
+        return None, f"capture {e.get('file')} was taken on other kernel sources ({e.get('kernel_source_sha')})"
+    return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), e.get("file")
+
+
+def sass_counts():
+    """profiles/sass_counts.json (written by build(): python -m paper_1802_05065_b200.sasscount --write)."""
+    try:
+        return json.load(open(os.path.join(PROFILES, "sass_counts.json")))["per_step"]
+    except (OSError, ValueError, KeyError):
+        return {}
+
+
+def sass_key(kind: str, params: dict) -> str:
+    return (f"{kind}_f{'32' if params['precision'] == 'fp32' else '64'}_{'ud' if params['model'] == 'underdamped' else 'od'}_"
+            f"{params['scheme']}_{'sin' if params['amp'] != 0.0 else 'nosin'}_{'ramp' if params['nu'] != 0.0 else 'const'}")
+
+
+def executed_per_step(counts: dict, params: dict, kernel: int):
+    """FP64 (FP32) pipe instructions the kernel that ran executes per trajectory step, from its SASS: the persistent
+    kernel's step loop, or consumer loop + producer loop of the specialised kernel."""
+    cls = "fp32" if params["precision"] == "fp32" else "fp64"
+    if kernel == 2:
+        e = counts.get(sass_key("specialised", params))
+        return None if not e else round(e["consumer_loop"][cls] + e["producer_loop"][cls], 2)
+    e = counts.get(sass_key("persistent", params))
+    return None if not e else e["step_loop"][cls]
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -124,25 +173,44 @@ def resolve_workload(fpt, name: str):
     return fpt.workload(name), None
 
 
+def config_dict(args, w, n_traj: int) -> dict:
+    """The `config` object of the JSON line: the same in both arms (ours / reference), world size excluded."""
+    return {"workload": f"{args.workload}: BASELINE.json configs[{int(args.workload[1]) - 1}]"
+                        + (" parameters, scaled twin" if args.workload in TWINS else ""), "n_traj_per_gpu": n_traj,
+            "seed": w["seed"], "t_max": w["t_max"], "params": {k2: v for k2, v in w["params"].items()},
+            "l2": "no input arrays (inputs are generated in-kernel from seed and id); 256 MiB written between timed steps",
+            "parallelism": "independent id ranges, one per GPU, no collective"}
+
+
+def bench_n_traj(args, w, n_twin):
+    n_traj = n_twin or w["n_traj"]
+    if args.workload in ("c3", "c4", "c5"):       # full configs take minutes: bench them on a fixed id range
+        n_traj = min(n_traj, 1 << 16)
+    if args.n_traj > 0:
+        n_traj = args.n_traj
+    return n_traj
+
+
 def run_reference(args, rank: int):
     """--impl reference: the oracle on the host cores (rank 0 only)."""
     if rank != 0:
         return
     import paper_1802_05065_b200 as fpt
-    w, _ = resolve_workload(fpt, args.workload)
+    w, n_twin = resolve_workload(fpt, args.workload)
+    n_traj = bench_n_traj(args, w, n_twin)
     per_step_budget = max(1.0, min(15.0, 90.0 / max(1, args.steps + args.warmup)))
     rates, esc, ids, secs = [], [], 0, 0.0
     cores = host_cores()
     for i in range(args.warmup + args.steps):
-        r, e, n, dt, cores = oracle_rate(w, per_step_budget, w["n_traj"], first_id=0)
+        r, e, n, dt, cores = oracle_rate(w, per_step_budget, n_traj, first_id=0)
         if i >= args.warmup:
             rates.append(r); esc.append(e); ids = n; secs += dt
     value = statistics.mean(rates)
-    sample = f"ids [0,{ids}) of {w['n_traj']} per step, OpenMP over trajectories, {cores} threads"
+    sample = f"ids [0,{ids}) of the {n_traj} of the config per step, OpenMP over trajectories, {cores} threads"
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * secs / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64" if w["params"]["precision"] == "fp64" else "f32", "data": "synthetic",
-            "config": {"workload": args.workload, "n_traj_per_step": ids},
+            "config": config_dict(args, w, n_traj), "oracle_ids_per_step": ids,
             "escapes_per_s": statistics.mean(esc),
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -151,20 +219,18 @@ def run_reference(args, rank: int):
 
 
 # ------------------------------------------------------------------------------------------------------------------
-def time_workload(fpt, torch, w, n_traj, steps, warmup, flush, first_id=0, hist=False):
-    """Device-timed steps of one workload; returns dict(ms list, stats of the last step, outputs)."""
+def time_workload(fpt, torch, w, n_traj, steps, warmup, flush, first_id=0, hist=False, opts=None):
+    """Device-timed steps of one workload through fpt_simulate_ex; returns dict(ms list, this call's statistics, outputs)."""
     p = fpt.make_params(**dict(w["params"], first_id=first_id))
     out = fpt.binding._alloc_outputs(n_traj)
-    counts = None
+    d_stats = fpt.alloc_stats()
+    h = None
     if hist and w.get("hist"):
         of, lo, hi, nb = w["hist"]
-        counts = torch.zeros(nb + 2, dtype=torch.int64, device="cuda")
+        h = (of, lo, hi, nb, torch.zeros(nb + 2, dtype=torch.int64, device="cuda"))
 
     def one():
-        if counts is not None:
-            fpt.simulate_hist(p, n_traj, w["seed"], w["t_max"], lo, hi, nb, hist_of=of, counts=counts, out=out)
-        else:
-            fpt.simulate(p, n_traj, w["seed"], w["t_max"], out=out)
+        fpt.simulate_ex(p, n_traj, w["seed"], w["t_max"], hist=h, opts=opts, stats=d_stats, out=out)
 
     for _ in range(warmup):
         one()
@@ -179,7 +245,7 @@ def time_workload(fpt, torch, w, n_traj, steps, warmup, flush, first_id=0, hist=
         e1.record()
         e1.synchronize()
         ms.append(e0.elapsed_time(e1))
-    return {"ms": ms, "stats": fpt.last_stats(), "out": out}
+    return {"ms": ms, "stats": fpt.read_stats(d_stats), "out": out}
 
 
 def main():
@@ -194,6 +260,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-traj", type=int, default=0, help="override the trajectories per step (0 = the config's own count)")
     ap.add_argument("--no-extra", action="store_true", help="skip the throughput-shaped extra workloads and the CPU baseline")
+    ap.add_argument("--no-stated", action="store_true", help="skip the two stated-parameter legs (c3, c5: ~45 s together)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -218,11 +285,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     w, n_twin = resolve_workload(fpt, args.workload)
-    n_traj = n_twin or w["n_traj"]
-    if args.workload in ("c3", "c4", "c5"):       # full configs take minutes: bench them on a fixed id range
-        n_traj = min(n_traj, 1 << 16)
-    if args.n_traj > 0:
-        n_traj = args.n_traj
+    n_traj = bench_n_traj(args, w, n_twin)
     n64 = w["n64_ref"]
     fp32 = w["params"]["precision"] == "fp32"
     flush = torch.zeros(256 << 20, dtype=torch.uint8, device="cuda")     # 256 MiB > 126 MB L2
@@ -282,50 +345,73 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * dev_s / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32" if fp32 else "f64", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: BASELINE.json configs[{int(args.workload[1]) - 1}]"
-                               + (" parameters, scaled twin" if args.workload in TWINS else ""), "n_traj_per_gpu": n_traj,
-                   "seed": w["seed"], "t_max": w["t_max"], "params": {k2: v for k2, v in w["params"].items()},
-                   "l2": "no input arrays (inputs are generated in-kernel from seed and id); 256 MiB written between timed steps",
-                   "parallelism": f"independent id ranges x{world}, no collective"},
+        "config": config_dict(args, w, n_traj),
         "escapes_per_s": escaped_all * args.steps / dev_s,
         "censored": int(st["n_censored"]), "lane_efficiency": st["lane_efficiency"],
-        "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"]},
+        "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"],
+                   "kernel": fpt.binding.KERNEL[st["kernel"]]},
         "wall_s_timed_region": t_wall, "ms_each_step": [round(x, 3) for x in res["ms"]],
         "e2e": {"value": useful_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 96,
                 "d2h_bytes_per_step": n_traj * 20, "api": "fpt_simulate_host (pinned host outputs; inputs = 96-byte fpt_params)"},
-        "gpu_launches": args.steps,             # one persistent-kernel launch per step (plus a memset and a 64-byte D2D copy)
+        "gpu_launches": 2 * args.steps,         # per step: the integrator kernel + the 1-thread statistics export (and a 128-byte memset)
         "clocks": clocks,
     }
     per_gpu_rate = (useful * args.steps / (sum(res["ms"]) * 1e-3))
+    counts = sass_counts()
+    n_exec = executed_per_step(counts, w["params"], st["kernel"])
+    traffic, traffic_src = ncu_traffic(args.workload, n_traj)
+    cls = "FP32" if fp32 else "FP64"
     line["roofline"] = {
         "bound": "alu", "achieved": per_gpu_rate * n64 / 1e9, "peak": peak / 1e9,
-        "unit": "G FP32 thread-instr/s" if fp32 else "G FP64 thread-instr/s",
+        "unit": f"G {cls} thread-instr/s",
         "frac": per_gpu_rate * n64 / peak,
-        "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (args.workload == "c2" and n_traj == 100000) else None,
-        "note": f"achieved = steps/s x {n64} reference {'FP32' if fp32 else 'FP64'}-pipe instructions per step (SURVEY 8(a)); peak = "
+        "traffic": traffic, "traffic_source": traffic_src,
+        "note": f"achieved = steps/s x {n64} reference {cls}-pipe instructions per step (SURVEY 8(a)); peak = "
                 f"{'FFMA' if fp32 else 'DFMA'} chains measured live by fpt_fp{'32' if fp32 else '64'}_peak after 1 s of load "
-                f"(SM clock seen {clk_hz / 1e6:.0f} MHz); MEASURED_PEAKS.json has no {'FP32' if fp32 else 'FP64'} figure",
+                f"(SM clock seen {clk_hz / 1e6:.0f} MHz); MEASURED_PEAKS.json has no {cls} figure",
         "hbm_bytes_per_step_algorithmic": n_traj * 20,
-        "fp64_instr_per_step_in_sass": {"c1": 30.9, "c2": 72.9, "c3": 74.9, "c5": 47.9}.get(args.workload),
+        # what the kernel that ran really executes per step (profiles/sass_counts.json, from cuobjdump -sass at build time)
+        "instr_per_step_executed": n_exec,
+        "frac_executed": None if n_exec is None else per_gpu_rate * n_exec / peak,
+        "kernel_source_sha": kernel_source_sha(),
     }
 
     if rank == 0 and world == 1 and not args.no_extra:
-        # ---- throughput-shaped workloads (same parameters as the configs, id ranges sized to fill the GPU for ~0.1-1 s)
+        # ---- throughput-shaped workloads: (i) the configs' parameters with the ramp rate / temperature changed so that a
+        # step lasts ~0.1-0.3 s (twins), (ii) configs 3 and 5 at their STATED parameters on a bounded id range (one timed
+        # step each, ~15-30 s): the numbers behind the 60 % target, timed by whoever runs this file
         extra = {}
-        shapes = [("c2_x42", "c2", dict(), 1 << 22, False),
-                  ("c3_fast_ramp",) + TWINS["c3_fast"] + (True,),
-                  ("c5_T0.1",) + TWINS["c5_T0.1"] + (False,),
-                  ("c4_fast_ramp",) + TWINS["c4_fast"] + (False,)]
-        for name, base, ov, n, hist in shapes:
+        shapes = [("c2_x42", "c2", dict(), 1 << 22, False, 3, None),
+                  ("c3_fast_ramp",) + TWINS["c3_fast"] + (True, 3, None),
+                  ("c5_T0.1",) + TWINS["c5_T0.1"] + (False, 3, None),
+                  ("c4_fast_ramp",) + TWINS["c4_fast"] + (False, 3, None)]
+        if not args.no_stated:
+            # the full configs keep every SM full (10^6 and 4 x 10^6 trajectories); their samples here are launched the same
+            # way: one whole wave of config 3 (ramped: every trajectory lasts about as long, so a ragged last wave would idle
+            # the GPU for a whole trajectory), 2^17 ids of config 5 on the full config's 3 blocks of 128 threads per SM
+            full = fpt.launch_opts(block=128, blocks_per_sm=3, specialise=False)
+            wave = time_workload(fpt, torch, fpt.workload("c3", t_max=10.0), 1 << 20, 0, 1, None, 0)["stats"]
+            shapes += [("c3_stated_one_wave", "c3", dict(), wave["grid"] * wave["block"], True, 1, None),
+                       ("c5_stated_ids_0_131072", "c5", dict(), 1 << 17, False, 1, full)]
+        for name, base, ov, n, hist, reps, opts in shapes:
             ww = fpt.workload(base, **ov)
-            r = time_workload(fpt, torch, ww, n, 3, 1, flush, 0, hist=hist)
+            if reps > 1:
+                r = time_workload(fpt, torch, ww, n, reps, 1, flush, 0, hist=hist, opts=opts)
+            else:                                   # long step: warm the kernel up on the same ids with the cap cut to 1e-4 of it
+                time_workload(fpt, torch, fpt.workload(base, t_max=ww["t_max"] * 1e-4), n, 0, 1, None, 0, hist=hist, opts=opts)
+                r = time_workload(fpt, torch, ww, n, 1, 0, flush, 0, hist=hist, opts=opts)
             sec = statistics.median(r["ms"]) * 1e-3
             stx = r["stats"]
             is32 = ww["params"]["precision"] == "fp32"
             pk = peak if is32 == fp32 else (fpt.fp32_peak if is32 else fpt.fp64_peak)(0.5)[0]
-            extra[name] = {"n_traj": n, "overrides": ov, "steps_per_s": stx["useful_steps"] / sec, "escapes_per_s": stx["n_escaped"] / sec,
+            nx = executed_per_step(counts, ww["params"], stx["kernel"])
+            rate = stx["useful_steps"] / sec
+            extra[name] = {"n_traj": n, "overrides": ov, "steps_per_s": rate, "escapes_per_s": stx["n_escaped"] / sec,
                            "ms": sec * 1e3, "censored": stx["n_censored"], "lane_efficiency": stx["lane_efficiency"],
-                           "roofline_frac": stx["useful_steps"] / sec * ww["n64_ref"] / pk, "n_ref_per_step": ww["n64_ref"],
+                           "roofline_frac": rate * ww["n64_ref"] / pk, "n_ref_per_step": ww["n64_ref"],
+                           "instr_per_step_executed": nx, "frac_executed": None if nx is None else rate * nx / pk,
+                           "launch": {"grid": stx["grid"], "block": stx["block"], "check_every": stx["check_every"],
+                                      "kernel": fpt.binding.KERNEL[stx["kernel"]]},
                            "dtype": "f32" if is32 else "f64"}
         line["extra_workloads"] = extra
         # ---- the oracle as it stands on the host cores, bounded sample of the same workload

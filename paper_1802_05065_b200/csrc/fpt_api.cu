@@ -289,13 +289,21 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     const size_t hist_bytes = with_hist ? (size_t)(hist->nbins + 2) * sizeof(unsigned int) : 0;
     const long long unit = 128LL * sms;                         // one warp per SM sub-partition everywhere
     // ---- which kernel.  The specialised kernel (consumers integrate, producers generate the normals) is for launches
-    // that cannot fill the GPU: with fewer than two warps of trajectories in flight per sub-partition a warp advances at
-    // the latency of its own instruction stream, and splitting that stream over warps shortens it.  Constant bias: the
-    // persistent kernel would keep n_traj / 5 trajectories in flight (below); ramped: all of them.
+    // that cannot fill the GPU: a warp that runs (nearly) alone advances at the latency of its own instruction stream, and
+    // splitting that stream over two warps on different sub-partitions shortens it (measured on B200, clk per step of a
+    // lone warp, persistent -> specialised: Heun underdamped 247 -> 184, Heun overdamped 360 -> 310, Euler overdamped
+    // 210 -> 172, Euler underdamped 178 -> 170, fp32 Heun underdamped 119 -> 91).  Up to two consumers per SM every
+    // consumer has a sub-partition to itself and every variant gains (10-25 % at 5000 trajectories); with four per SM only
+    // the fp64 Heun variants still gain (2-6 %), the others lose.  Trajectories in flight: the persistent kernel would
+    // keep n_traj / 5 of a constant-bias job in flight (below), all of a ramped one.
     const bool explicit_geometry = cfg.block > 0 || cfg.blocks_per_sm > 0;
-    const long long in_flight = ramp ? n_traj : n_traj / 5;
+    // consumers per SM wanted: all trajectories of a ramped job, a fifth of a constant-bias job but at least two
+    // consumers' worth (below that every consumer is alone on its sub-partition anyway)
+    const long long lanes_wanted = ramp ? n_traj : std::max<long long>(n_traj / 5, std::min<long long>(n_traj, 64LL * sms));
+    const long long nc_wanted = (lanes_wanted + 32LL * sms - 1) / (32LL * sms);
+    const bool spec_pays = nc_wanted <= 2 || (nc_wanted <= 8 && !fp32 && p->scheme == FPT_SCHEME_HEUN);
     const bool spec = amp && cfg.schedule == FPT_SCHEDULE_DYNAMIC && cfg.specialise >= 0 &&
-                      (cfg.specialise == 1 || (!explicit_geometry && in_flight < 2 * unit));
+                      (cfg.specialise == 1 || (!explicit_geometry && spec_pays));
     const void* fn = nullptr;
     size_t smem = hist_bytes;
     long long blocks = 0;
@@ -303,10 +311,8 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
       size_t fixed = 0, chan = 0;
       fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &fixed, &chan)
                 : specialised_kernel_f64(p->model, p->scheme, ramp, &fixed, &chan);
-      int NC = cfg.consumers > 0 ? cfg.consumers : 4;
+      int NC = cfg.consumers > 0 ? cfg.consumers : (int)std::min<long long>(4, std::max<long long>(1, nc_wanted));
       const int NP = cfg.producers > 0 ? cfg.producers : 1;
-      // few trajectories: fewer consumers per block, so that every SM gets some
-      while (cfg.consumers == 0 && NC > 1 && (long long)(NC - 1) * 32 * sms >= n_traj) --NC;
       P.spec_consumers = NC;
       P.spec_producers = NP;
       // a consumer must not share its SM sub-partition with a producer (fpt_specialised.cuh): with one producer each and

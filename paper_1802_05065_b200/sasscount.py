@@ -141,12 +141,19 @@ def count() -> dict:
     return table
 
 
+def write(table=None) -> Path:
+    """profiles/sass_counts.json"""
+    table = count() if table is None else table
+    OUT.parent.mkdir(exist_ok=True)
+    OUT.write_text(json.dumps({"command": "python -m paper_1802_05065_b200.sasscount --write  (cuobjdump -sass of libfpt_b200.so)",
+                               "per_step": table}, indent=1, sort_keys=True) + "\n")
+    return OUT
+
+
 def main():
     t = count()
     if "--write" in sys.argv:
-        OUT.parent.mkdir(exist_ok=True)
-        OUT.write_text(json.dumps({"command": "python -m paper_1802_05065_b200.sasscount --write  (cuobjdump -sass of libfpt_b200.so)",
-                                   "per_step": t}, indent=1, sort_keys=True) + "\n")
+        write(t)
     for k in sorted(t):
         e = t[k]
         for loop in ("step_loop", "consumer_loop", "producer_loop"):

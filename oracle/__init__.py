@@ -18,7 +18,7 @@ _SRC = _HERE / "fpt_oracle.cpp"
 _LIB = _HERE / "libfpt_oracle.so"
 
 MODEL = {"overdamped": 0, "underdamped": 1}
-SCHEME = {"em": 0, "heun": 1}
+SCHEME = {"em": 0, "heun": 1, "paper": 2}    # "paper": Alg. 1 / Alg. 3 as printed (gamma_k before the step, strict >)
 PRECISION = {"fp64": 0, "fp32": 1}
 
 

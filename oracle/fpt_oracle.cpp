@@ -275,7 +275,10 @@ extern "C" {
 struct oracle_params {
   int32_t model;        // 0 overdamped: dphi = (gamma(t) - amp sin phi) dt + sqrt(2 temperature) dW
                         // 1 underdamped: phi'' + alpha phi' + amp sin phi = gamma(t) + sqrt(2 alpha temperature) xi
-  int32_t scheme;       // 0 Euler-Maruyama (paper's Euler), 1 stochastic Heun
+  int32_t scheme;       // 0 Euler-Maruyama (paper's Euler), 1 stochastic Heun,
+                        // 2 the paper's kernels AS PRINTED (Alg. 1 / Alg. 3): Euler with the bias
+                        //   gamma_k = gamma0 + dgamma*k taken BEFORE the step (Alg. 3 line 13 precedes lines 14-15) and the
+                        //   strict comparison phi_k > th (Alg. 1 line 12, Alg. 3 line 16); reading R17
   int32_t precision;    // 0 fp64 state, 1 fp32 state + Kahan-compensated time
   int32_t reserved;
   double alpha, temperature, amp, gamma0, nu, phi0, v0, threshold, dt;
@@ -350,10 +353,22 @@ traj_result run_f64(const oracle_params& p, const derived& d, normal_source& ns,
   traj_result res{1, d.n_cap, phi, v};
   if (trace_len > 0) { trace_phi[0] = phi; if (trace_v) trace_v[0] = v; }
   if (phi != phi) { res.status = 2; res.k_end = 0; return res; }
-  if (phi >= thr) { res.status = 0; res.k_end = 0; return res; }           // O7: check at k = 0
+  // scheme 2 compares strictly (paper: "if phi_k > th"); schemes 0 and 1 with >= (reading R7)
+  auto crossed = [&](double x) { return p.scheme == 2 ? (x > thr) : (x >= thr); };
+  if (crossed(phi)) { res.status = 0; res.k_end = 0; return res; }         // O7: check at k = 0
   for (uint64_t k = 1; k <= d.n_cap; ++k) {
     const double z = ns.next64(k);
-    if (p.model == 0) {
+    if (p.scheme == 2) {                   // the paper's Euler as printed: gamma_k, not gamma_{k-1}, in step k
+      if (p.model == 0) {
+        const double f = F(phi, k);
+        phi = std::fma(sigma, z, std::fma(f, dt, phi));
+      } else {                             // Alg. 3 lines 13-15 (Alg. 1 lines 11-12 when dgamma = 0): both from the OLD state
+        const double a = std::fma(-alpha, v, F(phi, k));
+        const double phin = std::fma(v, dt, phi);
+        const double vn = std::fma(sigma, z, std::fma(a, dt, v));
+        phi = phin; v = vn;
+      }
+    } else if (p.model == 0) {
       if (p.scheme == 0) {                 // Euler-Maruyama, overdamped
         const double f = F(phi, k - 1);
         phi = std::fma(sigma, z, std::fma(f, dt, phi));
@@ -381,7 +396,7 @@ traj_result run_f64(const oracle_params& p, const derived& d, normal_source& ns,
     }
     if (k < trace_len) { trace_phi[k] = phi; if (trace_v) trace_v[k] = v; }
     if (phi != phi) { res.status = 2; res.k_end = k; break; }
-    if (phi >= thr) { res.status = 0; res.k_end = k; break; }              // O7: first k with phi_k >= threshold
+    if (crossed(phi)) { res.status = 0; res.k_end = k; break; }            // O7: first k with phi_k >= threshold (> for scheme 2)
   }
   res.phi_end = phi; res.v_end = v;
   return res;
@@ -400,7 +415,8 @@ traj_result run_f32(const oracle_params& p, const derived& d, normal_source& ns,
   traj_result res{1, d.n_cap, phi, v};
   if (trace_len > 0) { trace_phi[0] = phi; if (trace_v) trace_v[0] = v; }
   if (phi != phi) { res.status = 2; res.k_end = 0; return res; }
-  if (phi >= thr) { res.status = 0; res.k_end = 0; return res; }
+  auto crossed = [&](float x) { return p.scheme == 2 ? (x > thr) : (x >= thr); };
+  if (crossed(phi)) { res.status = 0; res.k_end = 0; return res; }
   for (uint64_t k = 1; k <= d.n_cap; ++k) {
     const float z = ns.next32(k);
     const float g1 = ramp ? std::fmaf(nu, t, g0) : g0;
@@ -411,7 +427,17 @@ traj_result run_f32(const oracle_params& p, const derived& d, normal_source& ns,
       t = s;
     }
     const float g2 = ramp ? std::fmaf(nu, t, g0) : g0;
-    if (p.model == 0) {
+    if (p.scheme == 2) {                   // the paper's Euler as printed: the bias AFTER the time update (gamma_k)
+      if (p.model == 0) {
+        const float f = F(phi, g2);
+        phi = std::fmaf(sigma, z, std::fmaf(f, dt, phi));
+      } else {
+        const float a = std::fmaf(-alpha, v, F(phi, g2));
+        const float phin = std::fmaf(v, dt, phi);
+        const float vn = std::fmaf(sigma, z, std::fmaf(a, dt, v));
+        phi = phin; v = vn;
+      }
+    } else if (p.model == 0) {
       if (p.scheme == 0) {
         const float f = F(phi, g1);
         phi = std::fmaf(sigma, z, std::fmaf(f, dt, phi));
@@ -439,7 +465,7 @@ traj_result run_f32(const oracle_params& p, const derived& d, normal_source& ns,
     }
     if (k < trace_len) { trace_phi[k] = phi; if (trace_v) trace_v[k] = v; }
     if (phi != phi) { res.status = 2; res.k_end = k; break; }
-    if (phi >= thr) { res.status = 0; res.k_end = k; break; }
+    if (crossed(phi)) { res.status = 0; res.k_end = k; break; }
   }
   res.phi_end = phi; res.v_end = v;
   return res;
@@ -447,7 +473,7 @@ traj_result run_f32(const oracle_params& p, const derived& d, normal_source& ns,
 
 bool params_ok(const oracle_params* p, double t_max) {
   if (!p) return false;
-  if (p->model < 0 || p->model > 1 || p->scheme < 0 || p->scheme > 1 || p->precision < 0 || p->precision > 1) return false;
+  if (p->model < 0 || p->model > 1 || p->scheme < 0 || p->scheme > 2 || p->precision < 0 || p->precision > 1) return false;
   const double f[] = {p->alpha, p->temperature, p->amp, p->gamma0, p->nu, p->phi0, p->v0, p->threshold, p->dt, t_max};
   for (double x : f) if (!std::isfinite(x)) return false;
   if (!(p->dt > 0.0) || !(t_max > 0.0) || p->temperature < 0.0) return false;

@@ -64,13 +64,22 @@ def run(model, scheme, alpha, temperature, amp, gamma0, nu, phi0, v0, threshold,
     F = lambda ph, j: gam(j) - amp * mp.sin(ph)
     states = [(phi, v)]
     margin = abs(phi - thr)
-    if phi >= thr:
+    # scheme 2 = the paper's Alg. 1 / Alg. 3 as printed: Euler with gamma_k (line 13 of
+    # Alg. 3 comes before the update) and the strict test phi_k > th
+    crossed = (lambda x: x > thr) if scheme == 2 else (lambda x: x >= thr)
+    if crossed(phi):
         return 0, 0, states, margin
     cache = {}
     limit = n_cap if max_steps is None else min(n_cap, max_steps)
     for k in range(1, limit + 1):
         z = mpf(normals[k - 1]) if normals is not None else normal_for_step(seed, tid, k, cache)
-        if model == 0:
+        if scheme == 2:
+            if model == 0:
+                phi = phi + F(phi, k) * dt + sigma * z
+            else:
+                a = F(phi, k) - alpha * v
+                phi, v = phi + v * dt, v + a * dt + sigma * z
+        elif model == 0:
             if scheme == 0:
                 phi = phi + F(phi, k - 1) * dt + sigma * z
             else:
@@ -89,7 +98,7 @@ def run(model, scheme, alpha, temperature, amp, gamma0, nu, phi0, v0, threshold,
                 phi, v = phi + h2 * (v + vp), v + h2 * (a1 + a2) + sigma * z
         states.append((phi, v))
         margin = min(margin, abs(phi - thr))
-        if phi >= thr:
+        if crossed(phi):
             return 0, k, states, margin
     return 1, limit, states, margin
 

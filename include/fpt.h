@@ -45,10 +45,18 @@ extern "C" {
 
 #define FPT_MODEL_OVERDAMPED  0
 #define FPT_MODEL_UNDERDAMPED 1
-#define FPT_SCHEME_EM   0
-#define FPT_SCHEME_HEUN 1
+#define FPT_SCHEME_EM    0
+#define FPT_SCHEME_HEUN  1
+#define FPT_SCHEME_PAPER 2   /* the paper's kernels AS PRINTED (Alg. 1 lines 11-12, Alg. 3 lines 13-16):
+                                Euler with the bias gamma_k = gamma0 + dgamma*k taken BEFORE step k (schemes 0, 1: gamma_{k-1}) and
+                                the strict crossing test phi_k > threshold (schemes 0, 1: >=).  The paper's threshold pi - phi0
+                                (Alg. 1 line 5) is the caller's `threshold`.  Bit-exact against the oracle like schemes 0 and 1. */
 #define FPT_PREC_FP64 0
 #define FPT_PREC_FP32 1
+#define FPT_PREC_FP32_FAST 2 /* fp32 state, and the drift sine taken by the hardware (sin.approx / MUFU.SIN) as in the paper's single
+                                precision kernels.  Only with FPT_SCHEME_PAPER and amp != 0.  The hardware sine has
+                                no CPU twin: results are NOT bit-comparable with the oracle, only statistically (tests: two-sample KS
+                                against the fp32 oracle); everything else is the FPT_PREC_FP32 arithmetic. */
 
 #define FPT_STATUS_ESCAPED  0
 #define FPT_STATUS_CENSORED 1
@@ -59,8 +67,9 @@ extern "C" {
 typedef struct fpt_params {
   int32_t  model;        /* 0 overdamped : dphi = (gamma(t) - amp*sin phi) dt + sqrt(2*temperature) dW
                             1 underdamped: phi'' + alpha*phi' + amp*sin phi = gamma(t) + sqrt(2*alpha*temperature) xi (Eq. 9) */
-  int32_t  scheme;       /* 0 Euler-Maruyama (paper's Euler, Alg. 1 lines 11-12), 1 stochastic Heun */
-  int32_t  precision;    /* 0 fp64 state; 1 fp32 state + Kahan-compensated time (outputs stay fp64 functions of k_esc) */
+  int32_t  scheme;       /* 0 Euler-Maruyama (paper's Euler, Alg. 1 lines 11-12), 1 stochastic Heun, 2 FPT_SCHEME_PAPER */
+  int32_t  precision;    /* 0 fp64 state; 1 fp32 state + Kahan-compensated time (outputs stay fp64 functions of k_esc);
+                            2 FPT_PREC_FP32_FAST */
   int32_t  check_every;  /* K >= 1: poll/refill interval in steps.  NEVER changes results (the crossing test is per step,
                             PAPER.md:190).  Rounded up to a multiple of the steps per Philox block (2 fp64, 4 fp32).
                             0 = library default. */
@@ -69,7 +78,7 @@ typedef struct fpt_params {
   double   amp;          /* amplitude of sin phi; 0 => drifted Brownian motion with mu = gamma0 */
   double   gamma0, nu;   /* bias ramp gamma(t) = gamma0 + nu*t, used as gamma_k = fma(nu*dt, k, gamma0) */
   double   phi0, v0;     /* initial state (paper: arcsin(gamma), 0) */
-  double   threshold;    /* escape when phi >= threshold (paper: pi - phi0) */
+  double   threshold;    /* escape when phi >= threshold (> with FPT_SCHEME_PAPER; paper: pi - phi0) */
   double   dt;           /* step h */
   uint64_t first_id;     /* trajectory id of element 0 of the outputs (sharding); the Philox stream is keyed by (seed, id) */
 } fpt_params;

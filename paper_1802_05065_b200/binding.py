@@ -13,8 +13,8 @@ _HERE = Path(__file__).resolve().parent
 _LIB_PATH = _HERE / "libfpt_b200.so"
 
 MODEL = {"overdamped": 0, "underdamped": 1}
-SCHEME = {"em": 0, "heun": 1}
-PRECISION = {"fp64": 0, "fp32": 1}
+SCHEME = {"em": 0, "heun": 1, "paper": 2}
+PRECISION = {"fp64": 0, "fp32": 1, "fp32_fast": 2}
 HIST_OF = {"gamma": 0, "fpt": 1}
 SCHEDULE = {"dynamic": 0, "static": 1}
 

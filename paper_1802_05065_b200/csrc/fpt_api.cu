@@ -109,7 +109,9 @@ bool finite_all(const double* x, int n) {
 
 int validate(const fpt_params* p, int64_t n_traj, double t_max) {
   if (!p || n_traj < 0) return FPT_E_INVALID;
-  if (p->model < 0 || p->model > 1 || p->scheme < 0 || p->scheme > 1 || p->precision < 0 || p->precision > 1) return FPT_E_INVALID;
+  if (p->model < 0 || p->model > 1 || p->scheme < 0 || p->scheme > 2 || p->precision < 0 || p->precision > 2) return FPT_E_INVALID;
+  // the hardware-sine variant exists for the paper's own kernels only (single precision, Euler as printed, a sine to take)
+  if (p->precision == FPT_PREC_FP32_FAST && (p->scheme != FPT_SCHEME_PAPER || p->amp == 0.0)) return FPT_E_INVALID;
   if (p->check_every < 0) return FPT_E_INVALID;
   const double f[] = {p->alpha, p->temperature, p->amp, p->gamma0, p->nu, p->phi0, p->v0, p->threshold, p->dt, t_max};
   if (!finite_all(f, 10)) return FPT_E_INVALID;
@@ -163,8 +165,8 @@ void derive(const fpt_params& p, double t_max, uint64_t seed, KParams& P) {
   P.h2_f = (float)P.h2;
   P.first_id = p.first_id;
   P.n_cap = (unsigned long long)std::nearbyint(t_max / p.dt);
-  const int macro = p.precision == FPT_PREC_FP32 ? 4 : 2;
-  const unsigned long long long_cap = p.precision == FPT_PREC_FP32 ? kLongCap32 : kLongCap64;
+  const int macro = p.precision != FPT_PREC_FP64 ? 4 : 2;
+  const unsigned long long long_cap = p.precision != FPT_PREC_FP64 ? kLongCap32 : kLongCap64;
   int K = p.check_every > 0 ? p.check_every : (P.n_cap >= long_cap ? kDefaultKLong : kDefaultK);
   K = ((K + macro - 1) / macro) * macro;
   P.K = K;
@@ -273,9 +275,13 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
   P.ws = ws;
 
   int grid = 1, block = 128, kernel = FPT_KERNEL_FILL;
-  const bool fp32 = p->precision == FPT_PREC_FP32;
+  const bool fp32 = p->precision != FPT_PREC_FP64;
+  const bool fast_sine = p->precision == FPT_PREC_FP32_FAST;
   const int sms = ctx->sm_count;
-  const bool at_once_escaped = fp32 ? !((float)p->phi0 < (float)p->threshold) : !(p->phi0 < p->threshold);
+  // the crossing test applied to the initial state: >= (strict > for the paper's scheme), in the state's precision
+  const bool strict = p->scheme == FPT_SCHEME_PAPER;
+  const bool at_once_escaped = fp32 ? (strict ? !((float)p->phi0 <= (float)p->threshold) : !((float)p->phi0 < (float)p->threshold))
+                                    : (strict ? !(p->phi0 <= p->threshold) : !(p->phi0 < p->threshold));
   if (at_once_escaped || P.n_cap == 0) {
     block = 256;
     grid = (int)std::min<int64_t>((n_traj + block - 1) / block, (int64_t)sms * 8);
@@ -302,7 +308,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     const long long lanes_wanted = ramp ? n_traj : std::max<long long>(n_traj / 5, std::min<long long>(n_traj, 64LL * sms));
     const long long nc_wanted = (lanes_wanted + 32LL * sms - 1) / (32LL * sms);
     const bool spec_pays = nc_wanted <= 2 || (nc_wanted <= 8 && !fp32 && p->scheme == FPT_SCHEME_HEUN);
-    const bool spec = amp && cfg.schedule == FPT_SCHEDULE_DYNAMIC && cfg.specialise >= 0 &&
+    const bool spec = amp && !fast_sine && cfg.schedule == FPT_SCHEDULE_DYNAMIC && cfg.specialise >= 0 &&
                       (cfg.specialise == 1 || (!explicit_geometry && spec_pays));
     const void* fn = nullptr;
     size_t smem = hist_bytes;
@@ -332,7 +338,9 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
       if (blocks > needed) blocks = needed;
       kernel = FPT_KERNEL_SPECIALISED;
     } else {
-      fn = fp32 ? persistent_kernel_f32(p->model, p->scheme, amp, ramp) : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
+      fn = fast_sine ? persistent_kernel_f32_fast(p->model, ramp)
+           : fp32    ? persistent_kernel_f32(p->model, p->scheme, amp, ramp)
+                     : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
       rc = ensure_dynamic_smem(fn, smem, dev);
       if (rc != FPT_OK) return rc;
       auto max_blocks_per_sm = [&](int blk, int* out) -> cudaError_t {
@@ -892,7 +900,8 @@ int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max,
   TraceArgs T{id, trace_len, trace_phi, trace_v, out_status, (unsigned long long*)out_k_end};
   // the same State specialisation as the production launch of these parameters (R15 shortcuts included)
   const bool amp = p->amp != 0.0, ramp = p->nu != 0.0;
-  const void* fn = p->precision == FPT_PREC_FP32 ? trace_kernel_f32(p->model, p->scheme, amp, ramp)
+  const void* fn = p->precision == FPT_PREC_FP32_FAST ? trace_kernel_f32_fast(p->model, ramp)
+                   : p->precision == FPT_PREC_FP32    ? trace_kernel_f32(p->model, p->scheme, amp, ramp)
                                                  : trace_kernel_f64(p->model, p->scheme, amp, ramp);
   void* args[] = {(void*)&P, (void*)&T};
   FPT_CUDA(cudaLaunchKernel(fn, dim3(1), dim3(32), args, 0, (cudaStream_t)s));

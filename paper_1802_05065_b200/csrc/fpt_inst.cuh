@@ -18,4 +18,8 @@ const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* fix
 const void* trace_kernel_f64(int model, int scheme, bool amp, bool ramp);
 const void* trace_kernel_f32(int model, int scheme, bool amp, bool ramp);
 
+// fp32 state with the hardware sine: scheme 2 (the paper's kernels as printed) with amp != 0 only
+const void* persistent_kernel_f32_fast(int model, bool ramp);
+const void* trace_kernel_f32_fast(int model, bool ramp);
+
 }  // namespace fpt

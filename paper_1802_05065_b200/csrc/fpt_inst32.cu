@@ -9,4 +9,8 @@ const void* specialised_kernel_f32(int model, int scheme, bool ramp, size_t* fix
 }
 const void* trace_kernel_f32(int model, int scheme, bool amp, bool ramp) { return Inst<State32>::trace(model, scheme, amp, ramp); }
 
+// fp32 state with the hardware sine (FPT_PREC_FP32_FAST): the paper's scheme with a sine only
+const void* persistent_kernel_f32_fast(int model, bool ramp) { return Inst<State32Fast>::persistent_paper(model, ramp); }
+const void* trace_kernel_f32_fast(int model, bool ramp) { return Inst<State32Fast>::trace_paper(model, ramp); }
+
 }  // namespace fpt

@@ -1,4 +1,4 @@
-// fpt_inst_impl.cuh -- the lookup tables of fpt_inst.cuh for one state template (State64 or State32).
+// fpt_inst_impl.cuh -- the lookup tables of fpt_inst.cuh for one state template (State64, State32 or State32Fast).
 #pragma once
 #include "fpt_inst.cuh"
 #include "fpt_integrator.cuh"
@@ -26,23 +26,32 @@ struct Inst {
     if (a) return r ? tk<M, S, true, true>() : tk<M, S, true, false>();
     return r ? tk<M, S, false, true>() : tk<M, S, false, false>();
   }
+  template <int M, int S>
+  static const void* pick_s(bool r) { return r ? sk<M, S, true>() : sk<M, S, false>(); }
+
+  // scheme: 0 Euler-Maruyama, 1 stochastic Heun, 2 the paper's kernels as printed
   static const void* persistent(int model, int scheme, bool a, bool r) {
-    if (model == 0) return scheme == 0 ? pick_p<0, 0>(a, r) : pick_p<0, 1>(a, r);
-    return scheme == 0 ? pick_p<1, 0>(a, r) : pick_p<1, 1>(a, r);
+    if (model == 0) return scheme == 0 ? pick_p<0, 0>(a, r) : scheme == 1 ? pick_p<0, 1>(a, r) : pick_p<0, 2>(a, r);
+    return scheme == 0 ? pick_p<1, 0>(a, r) : scheme == 1 ? pick_p<1, 1>(a, r) : pick_p<1, 2>(a, r);
   }
   static const void* trace(int model, int scheme, bool a, bool r) {
-    if (model == 0) return scheme == 0 ? pick_t<0, 0>(a, r) : pick_t<0, 1>(a, r);
-    return scheme == 0 ? pick_t<1, 0>(a, r) : pick_t<1, 1>(a, r);
+    if (model == 0) return scheme == 0 ? pick_t<0, 0>(a, r) : scheme == 1 ? pick_t<0, 1>(a, r) : pick_t<0, 2>(a, r);
+    return scheme == 0 ? pick_t<1, 0>(a, r) : scheme == 1 ? pick_t<1, 1>(a, r) : pick_t<1, 2>(a, r);
   }
   static const void* specialised(int model, int scheme, bool r, size_t* fixed_bytes, size_t* channel_bytes) {
     *fixed_bytes = spec_pool_bytes();
     *channel_bytes = spec_channel_bytes<St<0, 0, true, true>>();      // depends on the precision only
-    if (model == 0) {
-      if (scheme == 0) return r ? sk<0, 0, true>() : sk<0, 0, false>();
-      return r ? sk<0, 1, true>() : sk<0, 1, false>();
-    }
-    if (scheme == 0) return r ? sk<1, 0, true>() : sk<1, 0, false>();
-    return r ? sk<1, 1, true>() : sk<1, 1, false>();
+    if (model == 0) return scheme == 0 ? pick_s<0, 0>(r) : scheme == 1 ? pick_s<0, 1>(r) : pick_s<0, 2>(r);
+    return scheme == 0 ? pick_s<1, 0>(r) : scheme == 1 ? pick_s<1, 1>(r) : pick_s<1, 2>(r);
+  }
+  // the paper's scheme only, with a sine (the hardware-sine variant): persistent kernel and tracer
+  static const void* persistent_paper(int model, bool r) {
+    if (model == 0) return r ? pk<0, 2, true, true>() : pk<0, 2, true, false>();
+    return r ? pk<1, 2, true, true>() : pk<1, 2, true, false>();
+  }
+  static const void* trace_paper(int model, bool r) {
+    if (model == 0) return r ? tk<0, 2, true, true>() : tk<0, 2, true, false>();
+    return r ? tk<1, 2, true, true>() : tk<1, 2, true, false>();
   }
 };
 

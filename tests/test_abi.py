@@ -53,6 +53,17 @@ def _good():
     return dict(fpt.workload("c2")["params"])
 
 
+def test_hardware_sine_precision_only_with_the_paper_scheme_and_a_sine(lib):
+    base = dict(_good(), precision="fp32_fast")
+    call = lambda kw: lib.fpt_simulate(C.byref(fpt.make_params(**kw)), 10, 1, 1.0, C.c_void_p(8), None, C.c_void_p(8), None)
+    assert call(dict(base, scheme="heun")) == -1 and call(dict(base, scheme="em")) == -1
+    assert call(dict(base, scheme="paper", amp=0.0)) == -1
+    assert call(dict(base, scheme=3)) == -1 and call(dict(_good(), precision=3)) == -1
+    import torch
+    if not torch.cuda.is_available():
+        assert call(dict(base, scheme="paper")) == -2          # valid: gets as far as the (absent) device
+
+
 @pytest.mark.parametrize("field,value", [("dt", 0.0), ("dt", -1.0), ("dt", math.nan), ("temperature", -0.1), ("alpha", -1.0),
                                          ("model", 2), ("scheme", -1), ("precision", 3), ("check_every", -1),
                                          ("gamma0", math.inf), ("threshold", math.nan)])

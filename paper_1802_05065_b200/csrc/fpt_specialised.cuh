@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
       const real* zb = zbuf + (size_t)(cseq & 1ull) * (kChunk * 32) + lane;
 #pragma unroll 8
       for (int s = 0; s < kChunk; ++s) {
-        st.step(P, zb[s * 32]);
+        st.template step<true>(P, zb[s * 32]);
         cap.observe(st, P);
       }
       ++cseq;

@@ -98,8 +98,6 @@ typedef struct fpt_stats {
   uint64_t migrations;         /* trajectories parked by a sparse warp and adopted by another (drain-phase compaction) */
   uint64_t helper_lane_steps;  /* 32 * (steps whose normals a tail-helper or producer warp generated for another warp);
                                   NOT part of issued_lane_steps                                            */
-  uint64_t respeculated_chunks;/* specialised kernel, Heun underdamped: 64-step chunks a consumer redid because its guess of
-                                  a sine's range reduction was wrong in some lane (results are unaffected)   */
 } fpt_stats;
 
 #define FPT_KERNEL_FILL        0   /* every trajectory decided at k = 0 (phi0 >= threshold) or by n_cap == 0: no integration */

@@ -36,8 +36,7 @@ class FptStats(C.Structure):
     _fields_ = [("n_traj", C.c_uint64), ("n_escaped", C.c_uint64), ("n_censored", C.c_uint64), ("n_nan", C.c_uint64),
                 ("useful_steps", C.c_uint64), ("issued_lane_steps", C.c_uint64), ("refill_atomics", C.c_uint64),
                 ("n_cap", C.c_uint64), ("grid", C.c_int32), ("block", C.c_int32), ("check_every", C.c_int32),
-                ("kernel", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64),
-                ("respeculated_chunks", C.c_uint64)]
+                ("kernel", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64)]
 
     def as_dict(self):
         d = {k: int(getattr(self, k)) for k, _ in self._fields_}

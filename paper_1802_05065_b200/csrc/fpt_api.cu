@@ -209,7 +209,6 @@ __global__ void fpt_export_stats_kernel(const DevStats* ws, fpt_stats geo, fpt_s
   geo.refill_atomics = ws->refill_atomics;
   geo.migrations = ws->migrations;
   geo.helper_lane_steps = ws->helper_lane_steps;
-  geo.respeculated_chunks = ws->respeculated_chunks;
   if (user) *user = geo;
   *slot = geo;
   *slot_ticket = ticket;

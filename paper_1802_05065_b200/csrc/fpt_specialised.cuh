@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
   __syncthreads();
 
   unsigned long long s_useful = 0, s_chunks = 0, s_help = 0;
-  unsigned s_esc = 0, s_cens = 0, s_nan = 0, s_atom = 0, s_mig = 0, s_respec = 0;
+  unsigned s_esc = 0, s_cens = 0, s_nan = 0, s_atom = 0, s_mig = 0;
 
   if (is_consumer) {
     // ================================================================================================ consumer
@@ -242,29 +242,10 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
       EscapeCapture cap;
       cap.reset();
       const real* zb = zbuf + (size_t)(cseq & 1ull) * (kChunk * 32) + lane;
-      bool redo = true;
-      if (S::kSpeculates) {                                 // fast path: guessed range reduction (State64::step_spec)
-        const S st0 = st;
-        bool bad = false;
-        st.spec_begin(P);
 #pragma unroll 8
-        for (int s = 0; s < kChunk; ++s) {
-          st.step_spec(P, zb[s * 32], bad);
-          cap.observe(st, P);
-        }
-        redo = __any_sync(0xffffffffu, bad && active);      // a wrong guess in a live lane: the whole warp redoes the chunk
-        if (redo) {
-          st = st0;
-          cap.reset();
-          ++s_respec;
-        }
-      }
-      if (redo) {
-#pragma unroll 8
-        for (int s = 0; s < kChunk; ++s) {
-          st.template step<true>(P, zb[s * 32]);
-          cap.observe(st, P);
-        }
+      for (int s = 0; s < kChunk; ++s) {
+        st.template step<true>(P, zb[s * 32]);
+        cap.observe(st, P);
       }
       ++cseq;
       ++s_chunks;
@@ -369,7 +350,6 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
       atomicAdd(&P.ws->n_nan, (unsigned long long)nn);
       atomicAdd(&P.ws->refill_atomics, (unsigned long long)s_atom);
       if (s_mig) atomicAdd(&P.ws->migrations, (unsigned long long)s_mig);
-      if (s_respec) atomicAdd(&P.ws->respeculated_chunks, (unsigned long long)s_respec);
     } else if (s_help) {
       atomicAdd(&P.ws->helper_lane_steps, s_help * (unsigned long long)(M * 32));
     }

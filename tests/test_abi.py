@@ -36,7 +36,7 @@ def test_exports_every_declared_symbol(lib):
 def test_struct_layouts(lib):
     assert C.sizeof(fpt.FptParams) == 96              # 4 x int32, 9 x double, 1 x uint64, no padding
     assert fpt.FptParams.first_id.offset == 88
-    assert C.sizeof(fpt.FptStats) == 104 and fpt.FptStats.respeculated_chunks.offset == 96
+    assert C.sizeof(fpt.FptStats) == 96
     assert fpt.FptStats.migrations.offset == 80 and fpt.FptStats.kernel.offset == 76
     assert C.sizeof(fpt.FptLaunchOpts) == 32 and fpt.FptLaunchOpts.producers.offset == 28
     assert C.sizeof(fpt.FptHist) == 32 and fpt.FptHist.out_counts.offset == 24

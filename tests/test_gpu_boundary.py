@@ -78,26 +78,6 @@ def test_specialised_kernel_every_layout_matches_the_oracle(name, w, n):
     assert saw_migration, "drain compaction between consumers never triggered"
 
 
-def test_consumer_range_reduction_guess_and_its_rollback():
-    """Heun underdamped consumers guess the range-reduction word of the predictor's sine one step ahead (State64::step_spec) and
-    redo a chunk whenever a live lane guessed wrong.  On config 2 that is a rare event; with a coarse step and violent noise
-    (|v' - vp| dt of order 1) it happens in most chunks.  Either way the outputs are the oracle's, bit for bit."""
-    calm = fpt.workload("c2", t_max=300.0)
-    out, st = _ex(calm, 3001, fpt.launch_opts(specialise=True))
-    _assert_oracle(out, _oracle(calm, 3001))
-    chunks = st["issued_lane_steps"] // (64 * 32)
-    assert st["respeculated_chunks"] < 0.01 * chunks, (st["respeculated_chunks"], chunks)
-    for ramp, precision in ((0.0, "fp64"), (1e-3, "fp64"), (1e-3, "fp32")):
-        wild = dict(params=dict(model="underdamped", scheme="heun", precision=precision, alpha=0.5, temperature=3.0, amp=1.0, gamma0=0.3,
-                                nu=ramp, phi0=0.0, v0=0.0, threshold=60.0, dt=0.3), seed=77, t_max=900.0, hist=None)
-        ora = _oracle(wild, 2000)
-        assert 0 < np.sum(ora["status"] == 0) and np.sum(ora["status"] == 1) > 0
-        for opts in (fpt.launch_opts(specialise=True), fpt.launch_opts(specialise=True, consumers=2, producers=2, max_blocks=3)):
-            out, st = _ex(wild, 2000, opts)
-            _assert_oracle(out, ora)
-            assert st["kernel"] == 2 and st["respeculated_chunks"] > 100, st
-
-
 def test_specialised_kernel_is_the_default_for_small_jobs_only():
     w = fpt.workload("c2", t_max=60.0)
     out, st = _ex(w, 4000)

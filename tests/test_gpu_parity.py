@@ -419,8 +419,9 @@ def test_concurrent_streams_and_host_threads():
 
 
 def test_random_geometries_poll_intervals_and_helper_settings_agree():
-    """Stress of the scheduling machinery (refill, parking / adoption, tail helper, lobby): 40 (FPT_STRESS_TRIALS) random launch geometries,
-    poll intervals and helper settings on workloads with escaped AND censored trajectories must all give the outputs of
+    """Stress of the scheduling machinery of BOTH kernels (refill, parking / adoption, tail helper, lobby; consumer / producer
+    hand-over, mailbox refill, consumer compaction): 40 (FPT_STRESS_TRIALS) random launch geometries, poll intervals, helper
+    settings and consumer / producer layouts on workloads with escaped AND censored trajectories must all give the outputs of
     the first run, bit for bit -- the outputs are a function of (params, seed, id) only."""
     rng = np.random.default_rng(99)
     for w, n in [(fpt.workload("c2", t_max=90.0), 5000), (fpt.workload("c5", temperature=0.12, t_max=250.0), 4000),
@@ -436,11 +437,20 @@ def test_random_geometries_poll_intervals_and_helper_settings_agree():
             fpt.set_launch(block, per_sm, max_blocks)
             fpt.set_tail_helper(helper)
             try:
-                out = run_gpu(w, n, check_every=K)
+                out = run_gpu(w, n, check_every=K, both=False)
             finally:
                 fpt.set_launch(0, 0, 0)
                 fpt.set_tail_helper(True)
             assert all(np.array_equal(a, b) for a, b in zip(out, ref)), (block, per_sm, max_blocks, K, helper)
+            # ... and a random layout of the warp-specialised kernel (consumers x producers, blocks per SM, grid cap)
+            nc, npr = int(rng.integers(1, 5)), int(rng.integers(1, 4))
+            if nc * (1 + npr) > 12:
+                npr = 12 // nc - 1
+            opts = fpt.launch_opts(specialise=True, consumers=nc, producers=npr, blocks_per_sm=int(rng.choice([0, 1, 2, 3])),
+                                   max_blocks=int(rng.choice([0, 1, 2, 5, 37, 148])))
+            f2, g2, s2 = fpt.simulate_ex(fpt.make_params(**dict(w["params"], check_every=K)), n, w["seed"], w["t_max"], opts=opts)
+            torch.cuda.synchronize()
+            assert all(np.array_equal(_np(a), b) for a, b in zip((f2, g2, s2), ref)), (nc, npr, opts.blocks_per_sm, opts.max_blocks)
 
 
 def test_calls_can_be_captured_in_a_cuda_graph():

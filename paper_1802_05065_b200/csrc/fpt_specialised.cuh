@@ -237,6 +237,7 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
         if (__all_sync(0xffffffffu, ok)) break;
         __nanosleep(20);
       }
+      __syncwarp();                                         // lanes >= NP did not read a counter themselves: order them behind the lanes that did
       __threadfence_block();
       // ---- kChunk steps (S3..S6), sticky per-step escape capture as in the persistent kernel
       EscapeCapture cap;
@@ -306,6 +307,7 @@ __global__ void __launch_bounds__(kSpecMaxThreads, 1) fpt_specialised_kernel(con
       }
       stop = __shfl_sync(0xffffffffu, stop, 0);
       if (stop) break;
+      __syncwarp();                                         // only lane 0 observed cons_seq: order the warp's mailbox reads behind it
       __threadfence_block();
       const unsigned long long c0 = *(volatile unsigned long long*)&ch->mail_c0[lane];
       const unsigned long long id = *(volatile unsigned long long*)&ch->mail_id[lane];

@@ -35,14 +35,20 @@ PROFILES = os.path.join(ROOT, "profiles")
 
 
 def kernel_source_sha() -> str:
-    """sha256 over the CUDA sources the kernels are built from: ties a stored measurement to the code it was taken on."""
+    """sha256 over the CUDA sources the kernels are built from, comments and blank lines stripped: ties a stored measurement to
+    the CODE it was taken on (rewording a comment does not invalidate a capture, changing a statement does)."""
     import hashlib
+    import re
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1802_05065_b200", "csrc")
     for name in sorted(os.listdir(csrc)):
         if name.endswith((".cu", ".cuh")):
+            text = open(os.path.join(csrc, name), encoding="utf-8").read()
+            text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+            text = re.sub(r"//[^\n]*", "", text)
+            code = "\n".join(line.rstrip() for line in text.splitlines() if line.strip())
             h.update(name.encode())
-            h.update(open(os.path.join(csrc, name), "rb").read())
+            h.update(code.encode())
     return h.hexdigest()[:16]
 
 

@@ -14,10 +14,10 @@
 // j + 1, step index there) in its mailbox slot BEFORE the consumer releases buffer j - 1; the producers read the mailbox
 // when they start a chunk, so chunk j + 1 already carries the new stream.  The lane idles for the one chunk in between
 // (64 steps; mean trajectory of config 2: 5690).
-// Measured on B200: a consumer alone on its SM sub-partition advances at 195 clk per step against 257 for
-// a warp that also generates its normals; a consumer that shares its sub-partition with a PRODUCER (which has the
-// instruction-level parallelism to keep the FP64 pipe busy) falls back to 270-285, one that shares it with another
-// consumer much less.  Hence the warp layout: consumers and producers sit on different sub-partitions.
+// Measured on B200, Heun underdamped fp64, clk per step: a consumer alone on its SM sub-partition 184,
+// against 247 for a warp that also generates its normals; a consumer that shares its sub-partition with a PRODUCER (which
+// has the instruction-level parallelism to keep the FP64 pipe busy) 272-286; two consumers sharing one 248.  Hence the warp
+// layouts: up to two consumers per SM each have a sub-partition to themselves, and consumers never share one with a producer.
 // Once the ids are exhausted the consumers of a block compact their lanes exactly like the warps of the persistent
 // kernel (park / adopt through shared memory), so a block is soon down to one consumer and one producer.
 // Stream positions and arithmetic are those of the persistent kernel, so the outputs are the same bits.

@@ -98,6 +98,7 @@ typedef struct fpt_stats {
   uint64_t migrations;         /* trajectories parked by a sparse warp and adopted by another (drain-phase compaction) */
   uint64_t helper_lane_steps;  /* 32 * (steps whose normals a tail-helper or producer warp generated for another warp);
                                   NOT part of issued_lane_steps                                            */
+  uint64_t time_slices;        /* time slicing: quanta after which a trajectory was set aside for a waiting one           */
 } fpt_stats;
 
 #define FPT_KERNEL_FILL        0   /* every trajectory decided at k = 0 (phi0 >= threshold) or by n_cap == 0: no integration */
@@ -128,6 +129,15 @@ typedef struct fpt_launch_opts {
                              the dynamic schedule; otherwise the persistent kernel runs.                                  */
   int32_t consumers;      /* specialised kernel: consumer warps per block, 1..4 (0 = default)                           */
   int32_t producers;      /* specialised kernel: producer warps per consumer, 1..3 (0 = default)                        */
+  int32_t time_slice;     /* persistent kernel, dynamic schedule, more trajectories than resident lanes: 0 = automatic (ramped
+                             jobs, whose trajectories are equally long, of one to three ragged "waves", and ramped fp32 jobs
+                             of 3 to 3.8 blocks of 128 per SM, which then run 3 blocks per SM), 1 = always, -1 = never.  Block b
+                             then owns the trajectories b, b + grid, ...; a lane sets its trajectory aside in device memory
+                             (32 B per trajectory + 8 B per ring entry, from the call's stream-ordered pool) after a quantum
+                             of >= 2048 steps while others of its block's are waiting and takes the one that has waited
+                             longest (round robin), so that all trajectories advance at the same rate and no ragged last
+                             wave idles the GPU.  Results are the same bits either way.                                  */
+  int32_t reserved;       /* must be 0 */
 } fpt_launch_opts;
 
 /* Fused histogram request of fpt_simulate_ex (as fpt_simulate_hist). */
@@ -161,7 +171,7 @@ int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double
  * receives this call's fpt_stats, written stream-ordered after the integration (valid once cuda_stream has been
  * synchronised).  Calls from any number of host threads on any number of streams are independent.
  * Additional FPT_E_INVALID: a bad field of opts (block not a multiple of 32 in 32..256, negative counts, unknown schedule,
- * consumers > 4, producers > 3) or of hist (as fpt_simulate_hist). */
+ * consumers > 4, producers > 3, reserved != 0) or of hist (as fpt_simulate_hist). */
 int fpt_simulate_ex(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
                     double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
                     const fpt_hist* hist, const fpt_launch_opts* opts, fpt_stats* d_stats, void* cuda_stream);

@@ -36,7 +36,8 @@ class FptStats(C.Structure):
     _fields_ = [("n_traj", C.c_uint64), ("n_escaped", C.c_uint64), ("n_censored", C.c_uint64), ("n_nan", C.c_uint64),
                 ("useful_steps", C.c_uint64), ("issued_lane_steps", C.c_uint64), ("refill_atomics", C.c_uint64),
                 ("n_cap", C.c_uint64), ("grid", C.c_int32), ("block", C.c_int32), ("check_every", C.c_int32),
-                ("kernel", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64)]
+                ("kernel", C.c_int32), ("migrations", C.c_uint64), ("helper_lane_steps", C.c_uint64),
+                ("time_slices", C.c_uint64)]
 
     def as_dict(self):
         d = {k: int(getattr(self, k)) for k, _ in self._fields_}
@@ -45,9 +46,10 @@ class FptStats(C.Structure):
 
 
 class FptLaunchOpts(C.Structure):
-    """struct fpt_launch_opts of include/fpt.h (32 bytes); all zero = the library's defaults."""
+    """struct fpt_launch_opts of include/fpt.h (40 bytes); all zero = the library's defaults."""
     _fields_ = [("block", C.c_int32), ("blocks_per_sm", C.c_int32), ("max_blocks", C.c_int32), ("schedule", C.c_int32),
-                ("tail_helper", C.c_int32), ("specialise", C.c_int32), ("consumers", C.c_int32), ("producers", C.c_int32)]
+                ("tail_helper", C.c_int32), ("specialise", C.c_int32), ("consumers", C.c_int32), ("producers", C.c_int32),
+                ("time_slice", C.c_int32), ("reserved", C.c_int32)]
 
 
 class FptHist(C.Structure):
@@ -152,11 +154,13 @@ def simulate(params: FptParams, n_traj: int, seed: int, t_max: float, out=None, 
 
 
 def launch_opts(block=0, blocks_per_sm=0, max_blocks=0, schedule="dynamic", tail_helper=None, specialise=None, consumers=0,
-                producers=0) -> FptLaunchOpts:
-    """fpt_launch_opts.  tail_helper / specialise: None = the library's default, True = on / always, False = off / never."""
+                producers=0, time_slice=None) -> FptLaunchOpts:
+    """fpt_launch_opts.  tail_helper / specialise / time_slice: None = the library's default, True = on / always, False = off /
+    never."""
     tri = lambda v: 0 if v is None else (1 if v else -1)
     sch = SCHEDULE[schedule] if isinstance(schedule, str) else int(schedule)
-    return FptLaunchOpts(block, blocks_per_sm, max_blocks, sch, tri(tail_helper), tri(specialise), consumers, producers)
+    return FptLaunchOpts(block, blocks_per_sm, max_blocks, sch, tri(tail_helper), tri(specialise), consumers, producers,
+                         tri(time_slice), 0)
 
 
 def alloc_stats(n=1):

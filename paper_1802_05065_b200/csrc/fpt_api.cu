@@ -127,6 +127,7 @@ int validate_opts(const fpt_launch_opts* o) {
   if (o->blocks_per_sm < 0 || o->blocks_per_sm > 64 || o->max_blocks < 0) return FPT_E_INVALID;
   if (o->schedule != FPT_SCHEDULE_DYNAMIC && o->schedule != FPT_SCHEDULE_STATIC) return FPT_E_INVALID;
   if (o->tail_helper < -1 || o->tail_helper > 1 || o->specialise < -1 || o->specialise > 1) return FPT_E_INVALID;
+  if (o->time_slice < -1 || o->time_slice > 1 || o->reserved != 0) return FPT_E_INVALID;
   if (o->consumers < 0 || o->consumers > kSpecMaxConsumersHost || o->producers < 0 || o->producers > kSpecMaxProducersHost)
     return FPT_E_INVALID;
   return FPT_OK;
@@ -209,18 +210,23 @@ __global__ void fpt_export_stats_kernel(const DevStats* ws, fpt_stats geo, fpt_s
   geo.refill_atomics = ws->refill_atomics;
   geo.migrations = ws->migrations;
   geo.helper_lane_steps = ws->helper_lane_steps;
+  geo.time_slices = ws->time_slices;
   if (user) *user = geo;
   *slot = geo;
   *slot_ticket = ticket;
 }
 
-struct WsGuard {            // the per-call workspace goes back to the pool on every path, stream ordered
+struct WsGuard {            // the per-call workspaces go back to the pool on every path, stream ordered
   DevStats* ws = nullptr;
+  void* slice = nullptr;    // time slicing: n_traj parking slots + the waiting ring
   cudaStream_t stream = nullptr;
   ~WsGuard() {
+    if (slice) (void)cudaFreeAsync(slice, stream);
     if (ws) (void)cudaFreeAsync(ws, stream);
   }
 };
+
+
 
 // Opt in to more than 48 KB of shared memory when a launch needs it (fused histograms of many bins next to the drain pool
 // and the tail helper's buffer; the specialised kernel's hand-over rings).  FPT_E_INVALID when it cannot fit at all.
@@ -313,6 +319,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     const void* fn = nullptr;
     size_t smem = hist_bytes;
     long long blocks = 0;
+    bool want_slice = cfg.time_slice == 1;
     if (spec) {
       size_t fixed = 0, chan = 0;
       fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &fixed, &chan)
@@ -368,6 +375,18 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
           int per_sm128 = 0;
           FPT_CUDA(max_blocks_per_sm(128, &per_sm128));
           if (per_sm128 < 1) return FPT_E_CUDA;
+          // Time slicing (fpt_integrator.cuh): equal-length trajectories that do not fill a whole number of waves.  Between
+          // one and three waves with the last one ragged by more than 5 %: slice at full occupancy (beyond three waves the
+          // spread of the escape times blends the waves by itself, measured on config 4's twin at 3.46 waves: slicing costs
+          // 2 % there).  fp32, between 3 and 3.8 blocks of 128 per SM (config 4: 3.46): 3 blocks per SM + slicing instead of
+          // 4 and 3 blocks side by side -- measured on B200, a sub-partition with 3 warps does 95 % of the work of one with
+          // 4, so 3 everywhere for n / (3 x 128 x #SM) "waves" beats waiting for the SMs that got 4 (0.509 -> 0.572).
+          if (ramp && cfg.time_slice >= 0 && cfg.schedule == FPT_SCHEDULE_DYNAMIC) {
+            const double f = (double)n_traj / (double)unit;
+            const double waves = f / (double)per_sm128;
+            if (waves > 1.0 && waves < 3.0 && std::ceil(waves) > 1.05 * waves) want_slice = true;
+            else if (fp32 && per_sm128 >= 4 && f > 3.0 && f < 3.8) { want_slice = true; units = 3; }
+          }
           units = std::min<long long>(units, per_sm128);
           if (!fp32 && units >= 2 && (units % 2) == 0) {          // fp64: pairs of 128 as one 256-thread block (compaction
                                                                   // works over more lanes; measured +3 %, fp32: -20 %)
@@ -388,6 +407,24 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     }
     if (cfg.max_blocks > 0 && blocks > cfg.max_blocks) blocks = cfg.max_blocks;
     grid = (int)blocks;
+    if (want_slice && !spec && cfg.schedule == FPT_SCHEDULE_DYNAMIC && (long long)grid * block < n_traj &&
+        (cfg.time_slice == 1 || P.n_cap >= (1ull << 15))) {
+      // quantum: a power of two of steps, a multiple of K, at least 2048 (a hand-over costs a warp about as much as ten
+      // steps) and at least 1/2048 of the cap
+      unsigned long long q = 2048;
+      while (q < (unsigned long long)P.K || q * 2048ull < P.n_cap) q <<= 1;
+      if ((q % (unsigned long long)P.K) != 0ull) q *= (unsigned long long)P.K;       // K not a power of two: any multiple will do
+      if ((q & (q - 1ull)) == 0ull) {
+        P.slice_cap = ((unsigned long long)n_traj + (unsigned long long)grid - 1ull) / (unsigned long long)grid;
+        const size_t slot_bytes = (size_t)n_traj * sizeof(ParkSlot);
+        const size_t ring_bytes = (size_t)grid * (size_t)P.slice_cap * sizeof(unsigned long long);
+        FPT_CUDA(cudaMallocFromPoolAsync(&guard.slice, slot_bytes + ring_bytes, ctx->mem, stream));
+        P.slice_slots = (ParkSlot*)guard.slice;
+        P.slice_ring = (unsigned long long*)((char*)guard.slice + slot_bytes);
+        FPT_CUDA(cudaMemsetAsync(P.slice_ring, 0, ring_bytes, stream));
+        P.slice_mask = q - 1ull;
+      }
+    }
     P.schedule = cfg.schedule;
     P.tail_helper = cfg.tail_helper >= 0 ? 1 : 0;
     void* args[] = {(void*)&P};

@@ -36,9 +36,9 @@ def test_exports_every_declared_symbol(lib):
 def test_struct_layouts(lib):
     assert C.sizeof(fpt.FptParams) == 96              # 4 x int32, 9 x double, 1 x uint64, no padding
     assert fpt.FptParams.first_id.offset == 88
-    assert C.sizeof(fpt.FptStats) == 96
+    assert C.sizeof(fpt.FptStats) == 104 and fpt.FptStats.time_slices.offset == 96
     assert fpt.FptStats.migrations.offset == 80 and fpt.FptStats.kernel.offset == 76
-    assert C.sizeof(fpt.FptLaunchOpts) == 32 and fpt.FptLaunchOpts.producers.offset == 28
+    assert C.sizeof(fpt.FptLaunchOpts) == 40 and fpt.FptLaunchOpts.producers.offset == 28 and fpt.FptLaunchOpts.time_slice.offset == 32
     assert C.sizeof(fpt.FptHist) == 32 and fpt.FptHist.out_counts.offset == 24
     assert fpt.version() >= 200
 
@@ -105,6 +105,7 @@ def test_invalid_call_arguments(lib):
     assert ex(fpt.FptLaunchOpts(consumers=5)) == -1
     assert ex(fpt.FptLaunchOpts(producers=4)) == -1
     assert ex(fpt.FptLaunchOpts(max_blocks=-1)) == -1
+    assert ex(fpt.FptLaunchOpts(time_slice=2)) == -1 and ex(fpt.FptLaunchOpts(reserved=1)) == -1
     assert ex(None, fpt.FptHist(0, 0, 0.0, 1.0, 8)) == -1
     assert ex(None, fpt.FptHist(2, 10, 0.0, 1.0, 8)) == -1
     assert ex(None, fpt.FptHist(0, 10, 0.0, 1.0, None)) == -1

@@ -78,6 +78,61 @@ def test_specialised_kernel_every_layout_matches_the_oracle(name, w, n):
     assert saw_migration, "drain compaction between consumers never triggered"
 
 
+def test_time_slicing_rotates_trajectories_without_changing_results():
+    """fpt_launch_opts.time_slice: with fewer lanes than trajectories, a lane sets its trajectory aside in device memory every
+    quantum (2048 steps or more) while others of its block's wait and takes the one that has waited longest.  A set-aside trajectory resumes from (phi, v[, t, c],
+    k) with its Philox position, ramp registers and Kahan pair rebuilt: results stay the oracle's bit for bit -- ramped and
+    constant bias, fp64 and fp32, with the fused histogram -- and the rotation really happens."""
+    cases = [
+        (fpt.workload("c3", nu=2e-4, t_max=1.05 / 2e-4), 700, True),                         # fp64 ramp, ~2.4e5 steps each
+        (fpt.workload("c4", nu=2e-5, t_max=0.55 / 2e-5), 900, True),                         # fp32 + Kahan time, ~3.6e5 steps
+        (fpt.workload("c2", t_max=400.0), 3000, False),                                      # constant bias: finishes and preemptions mix
+        (fpt.workload("c5", temperature=0.1, t_max=1500.0), 2500, False),                    # EM overdamped, some censored
+    ]
+    for w, n, hist in cases:
+        ora = _oracle(w, n)
+        for geo in (dict(block=64, blocks_per_sm=1, max_blocks=5), dict(block=128, blocks_per_sm=1, max_blocks=2),
+                    dict(block=256, blocks_per_sm=1, max_blocks=1)):
+            out, st = _ex(w, n, fpt.launch_opts(specialise=False, time_slice=True, **geo), hist=hist)
+            _assert_oracle(out, ora, w)
+            assert st["kernel"] == 1 and st["time_slices"] > 0, st
+            assert st["useful_steps"] == int(np.sum(ora["k"])) and st["n_censored"] == int(np.sum(ora["status"] == 1))
+        out, st = _ex(w, n, fpt.launch_opts(specialise=False, time_slice=False, block=64, blocks_per_sm=1, max_blocks=5), hist=hist)
+        _assert_oracle(out, ora, w)
+        assert st["time_slices"] == 0
+    # all trajectories resident: nothing ever waits, nothing is set aside
+    w = fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3)
+    out, st = _ex(w, 256, fpt.launch_opts(specialise=False, time_slice=True, block=128, blocks_per_sm=1))
+    _assert_oracle(out, _oracle(w, 256), None)
+    assert st["time_slices"] == 0
+
+
+def test_time_slicing_is_the_default_where_equal_length_trajectories_leave_a_ragged_wave():
+    """The library's own choice (fpt_launch_opts.time_slice = 0): ramped fp32 jobs of 3 to 3.8 blocks of 128 per SM -- config 4's
+    65 536 trajectories on 148 SMs -- run 3 blocks per SM with slicing; ramped jobs of 1 to 3 ragged waves slice at full
+    occupancy; constant-bias jobs and short caps never do.  Same bits as without."""
+    import torch
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    w4 = fpt.workload("c4", nu=1.5e-4, t_max=0.5 / 1.5e-4)                                    # ~6.7e4 steps each, cap 2^16 or more
+    n = int(3.46 * 128 * sms)
+    out, st = _ex(w4, n)
+    assert st["kernel"] == 1 and st["grid"] == 3 * sms and st["block"] == 128 and st["time_slices"] > 0, st
+    out0, st0 = _ex(w4, n, fpt.launch_opts(time_slice=False))
+    assert st0["time_slices"] == 0 and st0["grid"] > 3 * sms
+    assert all(np.array_equal(a, b) for a, b in zip(out, out0))
+    w3 = fpt.workload("c3", nu=1e-3, t_max=1050.0)                                            # fp64, 1.5 waves
+    _, full = _ex(fpt.workload("c3", nu=1e-1, t_max=10.5), 1 << 19)
+    lanes = full["grid"] * full["block"]
+    out, st = _ex(w3, lanes * 3 // 2)
+    assert st["time_slices"] > 0 and st["grid"] * st["block"] == lanes, st
+    out0, st0 = _ex(w3, lanes * 3 // 2, fpt.launch_opts(time_slice=False))
+    assert st0["time_slices"] == 0 and all(np.array_equal(a, b) for a, b in zip(out, out0))
+    _, st = _ex(w3, lanes * 5)                                                               # five waves: blends by itself
+    assert st["time_slices"] == 0
+    _, st = _ex(fpt.workload("c2", t_max=2000.0), lanes * 3 // 2)                            # constant bias: refill balances
+    assert st["time_slices"] == 0
+
+
 def test_specialised_kernel_is_the_default_for_small_jobs_only():
     w = fpt.workload("c2", t_max=60.0)
     out, st = _ex(w, 4000)

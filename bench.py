@@ -266,6 +266,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--n-traj", type=int, default=0, help="override the trajectories per step (0 = the config's own count)")
     ap.add_argument("--no-extra", action="store_true", help="skip the throughput-shaped extra workloads and the CPU baseline")
+    ap.add_argument("--no-time-slice", action="store_true", help="main workload: forbid time slicing (profiling the unsliced geometry)")
     ap.add_argument("--no-stated", action="store_true", help="skip the two stated-parameter legs (c3, c5: ~45 s together)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -306,12 +307,13 @@ def main():
 
     # ---- device-timed region: exactly K steps
     first_id = fpt.sharding.shard_range(n_traj * world, rank, world)[0]      # rank r integrates ids [r*n, (r+1)*n)
-    time_workload(fpt, torch, w, n_traj, 0, args.warmup, flush, first_id)          # warm-up
+    main_opts = fpt.launch_opts(time_slice=False) if args.no_time_slice else None
+    time_workload(fpt, torch, w, n_traj, 0, args.warmup, flush, first_id, opts=main_opts)          # warm-up
     sampler = ClockSampler(local_rank)
     barrier()
     sampler.start()
     t_wall0 = time.perf_counter()
-    res = time_workload(fpt, torch, w, n_traj, args.steps, 0, flush, first_id)
+    res = time_workload(fpt, torch, w, n_traj, args.steps, 0, flush, first_id, opts=main_opts)
     barrier()
     t_wall = time.perf_counter() - t_wall0
     clocks = sampler.stop()
@@ -355,7 +357,7 @@ def main():
         "escapes_per_s": escaped_all * args.steps / dev_s,
         "censored": int(st["n_censored"]), "lane_efficiency": st["lane_efficiency"],
         "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"],
-                   "kernel": fpt.binding.KERNEL[st["kernel"]]},
+                   "kernel": fpt.binding.KERNEL[st["kernel"]], "time_slices": st["time_slices"]},
         "wall_s_timed_region": t_wall, "ms_each_step": [round(x, 3) for x in res["ms"]],
         "e2e": {"value": useful_all * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 96,
                 "d2h_bytes_per_step": n_traj * 20, "api": "fpt_simulate_host (pinned host outputs; inputs = 96-byte fpt_params)"},
@@ -390,7 +392,9 @@ def main():
         shapes = [("c2_x42", "c2", dict(), 1 << 22, False, 3, None),
                   ("c3_fast_ramp",) + TWINS["c3_fast"] + (True, 3, None),
                   ("c5_T0.1",) + TWINS["c5_T0.1"] + (False, 3, None),
-                  ("c4_fast_ramp",) + TWINS["c4_fast"] + (False, 3, None)]
+                  ("c4_fast_ramp",) + TWINS["c4_fast"] + (False, 3, None),
+                  # config 4's own launch geometry (65 536 trajectories: 3.46 blocks of 128 per SM -> 3 per SM, time-sliced)
+                  ("c4_fast_ramp_stated_geometry",) + TWINS["c4_fast"][:2] + (1 << 16, False, 3, None)]
         if not args.no_stated:
             # the full configs keep every SM full (10^6 and 4 x 10^6 trajectories); their samples here are launched the same
             # way: one whole wave of config 3 (ramped: every trajectory lasts about as long, so a ragged last wave would idle
@@ -417,7 +421,7 @@ def main():
                            "roofline_frac": rate * ww["n64_ref"] / pk, "n_ref_per_step": ww["n64_ref"],
                            "instr_per_step_executed": nx, "frac_executed": None if nx is None else rate * nx / pk,
                            "launch": {"grid": stx["grid"], "block": stx["block"], "check_every": stx["check_every"],
-                                      "kernel": fpt.binding.KERNEL[stx["kernel"]]},
+                                      "kernel": fpt.binding.KERNEL[stx["kernel"]], "time_slices": stx["time_slices"]},
                            "dtype": "f32" if is32 else "f64"}
         line["extra_workloads"] = extra
         # ---- the oracle as it stands on the host cores, bounded sample of the same workload

@@ -39,6 +39,10 @@ int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t bl
  * product's value).  The counters are 64-bit; a test presets them just below 2^32 to run across the point where 32-bit
  * counters would wrap. */
 int fpt_dbg_set_helper_seq0(uint64_t seq0);
+/* Quantum of the time slicing (fpt_launch_opts.time_slice) for the calls the CALLING THREAD makes afterwards: a power of
+ * two of steps (it is raised to the call's poll interval K when smaller), 0 = the product's value (>= 2048).  A test
+ * sets 64 to drive thousands of hand-overs through a small job.  FPT_E_INVALID when not 0 or a power of two. */
+int fpt_dbg_set_slice_quantum(uint64_t steps);
 /* one trajectory (id) with its states recorded: trace_phi[k], trace_v[k] for k = 0..min(k_end, trace_len-1) (as double),
  * out_status[0], out_k_end[0]; entries past k_end are left untouched. */
 int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len,

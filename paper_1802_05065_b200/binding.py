@@ -90,6 +90,7 @@ _SIGNATURES = {
     "fpt_dbg_sincos_f32": [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p],
     "fpt_dbg_selfcheck": [C.c_uint64, C.c_uint64, C.c_int64, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_dbg_set_helper_seq0": [C.c_uint64],
+    "fpt_dbg_set_slice_quantum": [C.c_uint64],
     "fpt_dbg_trace": [C.POINTER(FptParams), C.c_uint64, C.c_uint64, C.c_double, C.c_int64, C.c_void_p, C.c_void_p,
                       C.c_void_p, C.c_void_p, C.c_void_p],
 }
@@ -352,6 +353,10 @@ def dbg_selfcheck(seed, id0, n_threads, blocks_per_thread, stream=None):
 
 def dbg_set_helper_seq0(seq0=0):
     _check(lib().fpt_dbg_set_helper_seq0(seq0), "fpt_dbg_set_helper_seq0")
+
+
+def dbg_set_slice_quantum(steps=0):
+    _check(lib().fpt_dbg_set_slice_quantum(steps), "fpt_dbg_set_slice_quantum")
 
 
 def dbg_trace(params: FptParams, seed, tid, t_max, trace_len, stream=None):

@@ -46,6 +46,7 @@ constexpr int kSpecMaxConsumersHost = 4, kSpecMaxProducersHost = 3;
 // Defaults of the calls that take no fpt_launch_opts: per THREAD (the deprecated fpt_set_* shims write them).
 thread_local fpt_launch_opts t_opts = {};
 thread_local unsigned long long t_dbg_seq0 = 0;
+thread_local unsigned long long t_dbg_slice_q = 0;
 
 constexpr int kSweepStreams = 8;
 constexpr int kLastSlots = 256;   // ring of "last call" statistics blocks per device (fpt_last_stats shim)
@@ -413,6 +414,10 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
       // steps) and at least 1/2048 of the cap
       unsigned long long q = 2048;
       while (q < (unsigned long long)P.K || q * 2048ull < P.n_cap) q <<= 1;
+      if (t_dbg_slice_q != 0ull) {                                  // test hook (fpt_dbg.h)
+        q = t_dbg_slice_q;
+        while (q < (unsigned long long)P.K) q <<= 1;
+      }
       if ((q % (unsigned long long)P.K) != 0ull) q *= (unsigned long long)P.K;       // K not a power of two: any multiple will do
       if ((q & (q - 1ull)) == 0ull) {
         P.slice_cap = ((unsigned long long)n_traj + (unsigned long long)grid - 1ull) / (unsigned long long)grid;
@@ -925,6 +930,11 @@ int fpt_dbg_selfcheck(uint64_t seed, uint64_t id0, int64_t n_threads, int32_t bl
 }
 int fpt_dbg_set_helper_seq0(uint64_t seq0) {
   t_dbg_seq0 = seq0;
+  return FPT_OK;
+}
+int fpt_dbg_set_slice_quantum(uint64_t steps) {
+  if (steps != 0 && (steps & (steps - 1)) != 0) return FPT_E_INVALID;
+  t_dbg_slice_q = steps;
   return FPT_OK;
 }
 int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max, int64_t trace_len, double* trace_phi,

@@ -111,6 +111,7 @@ def test_invalid_call_arguments(lib):
     assert ex(None, fpt.FptHist(0, 10, 0.0, 1.0, None)) == -1
     assert lib.fpt_simulate_ex(C.byref(p), 0, 1, 1.0, None, None, None, None, None, None, None) == 0
     assert lib.fpt_set_specialise(2, 0, 0) == -1 and lib.fpt_set_specialise(0, 0, 0) == 0
+    assert lib.fpt_dbg_set_slice_quantum(96) == -1 and lib.fpt_dbg_set_slice_quantum(64) == 0 and lib.fpt_dbg_set_slice_quantum(0) == 0
     assert lib.fpt_set_launch(48, 0, 0) == -1
     assert lib.fpt_set_launch(512, 0, 0) == -1
     assert lib.fpt_set_launch(128, 2, 0) == 0

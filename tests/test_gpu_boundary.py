@@ -100,6 +100,16 @@ def test_time_slicing_rotates_trajectories_without_changing_results():
         out, st = _ex(w, n, fpt.launch_opts(specialise=False, time_slice=False, block=64, blocks_per_sm=1, max_blocks=5), hist=hist)
         _assert_oracle(out, ora, w)
         assert st["time_slices"] == 0
+    # a quantum of 64 steps (test hook): tens of hand-overs per trajectory, every poll of a K = 64 launch
+    w, n, hist = cases[2]
+    ora = _oracle(w, n)
+    fpt.dbg_set_slice_quantum(64)
+    try:
+        out, st = _ex(w, n, fpt.launch_opts(specialise=False, time_slice=True, block=96, blocks_per_sm=1, max_blocks=3), hist=hist)
+    finally:
+        fpt.dbg_set_slice_quantum(0)
+    _assert_oracle(out, ora, w)
+    assert st["time_slices"] > 20 * n, st
     # all trajectories resident: nothing ever waits, nothing is set aside
     w = fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3)
     out, st = _ex(w, 256, fpt.launch_opts(specialise=False, time_slice=True, block=128, blocks_per_sm=1))

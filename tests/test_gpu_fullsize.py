@@ -99,7 +99,7 @@ def test_full_config(name):
     rec = {"config": name, "n_traj": n, "seed": w["seed"], "t_max": w["t_max"], "seconds": sec, "steps": st["useful_steps"],
            "steps_per_s": steps_per_s, "escapes_per_s": st["n_escaped"] / sec, "escaped": st["n_escaped"],
            "censored": st["n_censored"], "lane_efficiency": st["lane_efficiency"], "migrations": st["migrations"],
-           "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"]},
+           "launch": {"grid": st["grid"], "block": st["block"], "check_every": st["check_every"], "time_slices": st["time_slices"]},
            "roofline_frac": steps_per_s * w["n64_ref"] / peak, "n_ref_per_step": w["n64_ref"], "peak_inst_per_s": peak,
            "sm_clock_hz_seen": clk, "mean_steps": float(k.mean()), "min_steps": int(k.min()), "max_steps": int(k.max()),
            "hist": rec_hist, "oracle_sampled_ids": len(ids), "oracle_seconds": t_oracle, "oracle_cores": os.cpu_count(),

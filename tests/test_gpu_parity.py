@@ -420,7 +420,7 @@ def test_concurrent_streams_and_host_threads():
 
 def test_random_geometries_poll_intervals_and_helper_settings_agree():
     """Stress of the scheduling machinery of BOTH kernels (refill, parking / adoption, tail helper, lobby; consumer / producer
-    hand-over, mailbox refill, consumer compaction): 40 (FPT_STRESS_TRIALS) random launch geometries, poll intervals, helper
+    hand-over, mailbox refill, consumer compaction; time slicing): 40 (FPT_STRESS_TRIALS) random launch geometries, poll intervals, helper
     settings and consumer / producer layouts on workloads with escaped AND censored trajectories must all give the outputs of
     the first run, bit for bit -- the outputs are a function of (params, seed, id) only."""
     rng = np.random.default_rng(99)
@@ -442,6 +442,18 @@ def test_random_geometries_poll_intervals_and_helper_settings_agree():
                 fpt.set_launch(0, 0, 0)
                 fpt.set_tail_helper(True)
             assert all(np.array_equal(a, b) for a, b in zip(out, ref)), (block, per_sm, max_blocks, K, helper)
+            # ... the same geometry with time slicing forced, quantum 64 / 512 / 2048 steps (hand-overs through device memory
+            # mixed with finishes, refills of the block's own ids, parking and the tail helper)
+            quantum = int(rng.choice([64, 512, 2048]))
+            fpt.dbg_set_slice_quantum(quantum)
+            try:
+                opts = fpt.launch_opts(block=block, blocks_per_sm=per_sm, max_blocks=max_blocks, tail_helper=helper,
+                                       specialise=False, time_slice=True)
+                f1, g1, s1 = fpt.simulate_ex(fpt.make_params(**dict(w["params"], check_every=K)), n, w["seed"], w["t_max"], opts=opts)
+                torch.cuda.synchronize()
+            finally:
+                fpt.dbg_set_slice_quantum(0)
+            assert all(np.array_equal(_np(a), b) for a, b in zip((f1, g1, s1), ref)), (block, per_sm, max_blocks, K, helper, quantum)
             # ... and a random layout of the warp-specialised kernel (consumers x producers, blocks per SM, grid cap)
             nc, npr = int(rng.integers(1, 5)), int(rng.integers(1, 4))
             if nc * (1 + npr) > 12:

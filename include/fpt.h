@@ -42,6 +42,7 @@ extern "C" {
 #define FPT_OK          0
 #define FPT_E_INVALID (-1)   /* bad argument (see each function)                  */
 #define FPT_E_CUDA    (-2)   /* CUDA runtime failure (no device, alloc, launch)   */
+#define FPT_E_TOO_LARGE (-3) /* a size beyond an entry point's fixed maximum (fpt_simulate_noalloc); nothing enqueued */
 
 #define FPT_MODEL_OVERDAMPED  0
 #define FPT_MODEL_UNDERDAMPED 1
@@ -175,6 +176,28 @@ int fpt_simulate_hist(const fpt_params* p, int64_t n_traj, uint64_t seed, double
 int fpt_simulate_ex(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
                     double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
                     const fpt_hist* hist, const fpt_launch_opts* opts, fpt_stats* d_stats, void* cuda_stream);
+
+/* fpt_simulate for callers that must not allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): same arguments, same results bit for bit (Alg. 1 / Alg. 3; outputs are
+ * a function of (params, seed, id) only), but this entry point calls no cudaMalloc / cudaMallocAsync / cudaFree or any other
+ * allocating routine, on the first call or later.  It always runs the persistent kernel, and all the scratch memory that
+ * kernel needs -- the global id counter and statistics block, and the parking slots and waiting rings of time slicing
+ * (fpt_launch_opts.time_slice; used here for ramped jobs with more trajectories than resident lanes) -- lives in ONE
+ * file-scope device array of the library, 5.3 MB, which every GPU that loads the library holds until the process exits.
+ *   - Limit: n_traj <= FPT_NOALLOC_MAX_TRAJ, else FPT_E_TOO_LARGE (nothing is enqueued or written).  Otherwise argument
+ *     checks and FPT_E_INVALID as fpt_simulate.  No fused histogram, no launch options.
+ *   - d_stats: NULL, or a caller-owned DEVICE fpt_stats block written at the end of the call (as fpt_simulate_ex).
+ *     fpt_last_stats does not see these calls.
+ *   - The array is shared by every call and keeps the last call's contents; each call clears, on cuda_stream, what must start
+ *     at zero.  Calls that may OVERLAP ON THE GPU (different streams, several host threads) race on it and give wrong
+ *     results: issue them on one stream, or order them with events.  One array per device: calls on different GPUs are
+ *     independent.
+ *   - The first launch of a kernel in a process loads its code (CUDA lazy loading, done by the driver): make one warm-up
+ *     call before capturing a graph.  Asynchronous, stream-ordered like fpt_simulate. */
+#define FPT_NOALLOC_MAX_TRAJ 131072
+int fpt_simulate_noalloc(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max,
+                         double* out_fpt, double* out_gamma_at_escape, int32_t* out_status,
+                         fpt_stats* d_stats, void* cuda_stream);
 
 /* Histogram of values[i] over the entries with status[i] == 0 (status may be NULL: all entries):
  *   b = floor((x - lo) * (nbins/(hi-lo))) in fp64, the scale computed once; b < 0 -> under, b >= nbins -> over (x == hi is

@@ -67,6 +67,8 @@ _SIGNATURES = {
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_simulate_ex": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                         C.POINTER(FptHist), C.POINTER(FptLaunchOpts), C.c_void_p, C.c_void_p],
+    "fpt_simulate_noalloc": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
+                             C.c_void_p, C.c_void_p],
     "fpt_histogram": [C.c_void_p, C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_int32, C.c_void_p, C.c_void_p],
     "fpt_simulate_host": [C.POINTER(FptParams), C.c_int64, C.c_uint64, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p,
                           C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_void_p],
@@ -194,6 +196,22 @@ def simulate_ex(params: FptParams, n_traj: int, seed: int, t_max: float, hist=No
                                  C.byref(h) if h is not None else None, C.byref(opts) if opts is not None else None, sp,
                                  _stream(stream)), "fpt_simulate_ex")
     return fpt, gam, st
+
+
+NOALLOC_MAX_TRAJ = 131072       # FPT_NOALLOC_MAX_TRAJ
+
+
+def simulate_noalloc(params: FptParams, n_traj: int, seed: int, t_max: float, out, stats=None, stream=None):
+    """fpt_simulate_noalloc: `out` = (fpt f64, gamma f64 or None, status i32) CUDA tensors the CALLER allocated; stats as in
+    simulate_ex.  The library allocates nothing; calls that overlap on the GPU race on its one scratch array.  Returns out."""
+    fpt, gam, st = out
+    sp = C.c_void_p(0)
+    if stats is not None:
+        t, i = stats if isinstance(stats, tuple) else (stats, 0)
+        sp = C.c_void_p(t.data_ptr() + i * C.sizeof(FptStats))
+    _check(lib().fpt_simulate_noalloc(C.byref(params), n_traj, seed, t_max, _ptr(fpt), _ptr(gam), _ptr(st), sp, _stream(stream)),
+           "fpt_simulate_noalloc")
+    return out
 
 
 def simulate_hist(params: FptParams, n_traj: int, seed: int, t_max: float, lo: float, hi: float, nbins: int,

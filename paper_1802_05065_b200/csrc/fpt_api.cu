@@ -864,6 +864,7 @@ const char* fpt_strerror(int code) {
     case FPT_OK: return "ok";
     case FPT_E_INVALID: return "invalid argument";
     case FPT_E_CUDA: return g_last_cuda != cudaSuccess ? cudaGetErrorString(g_last_cuda) : "CUDA failure";
+    case FPT_E_TOO_LARGE: return "size beyond the fixed maximum of this entry point (fpt_simulate_noalloc: FPT_NOALLOC_MAX_TRAJ trajectories)";
     default: return "unknown error code";
   }
 }
@@ -956,3 +957,136 @@ int fpt_dbg_trace(const fpt_params* p, uint64_t seed, uint64_t id, double t_max,
 }
 
 }  // extern "C"
+
+// =================================================================================================================
+// fpt_simulate_noalloc (fpt.h): the persistent kernel with ALL its scratch memory in one file-scope device array, for callers
+// that must not allocate (no cudaMalloc / cudaMallocAsync / cudaFree / memory-pool call on this path, ever; it does not
+// touch device_ctx(), whose first call per device allocates).  The array is part of the library's image: every GPU that
+// loads the library holds it (5.3 MB) until the process exits.  It is shared by all calls and keeps the last call's
+// contents; what must start at zero (the counters, the ring entries this call will use) is cleared on the caller's stream
+// at the start of every call.  Two calls that overlap on the GPU would share the id counter and the parking slots: they race.
+namespace {
+
+constexpr unsigned long long kNoAllocMaxTraj = FPT_NOALLOC_MAX_TRAJ;
+constexpr unsigned long long kNoAllocMaxGrid = 1024;               // ceil(max n_traj / 128): never more lanes than trajectories
+constexpr size_t kNoAllocHeader = 512;                             // DevStats (128 B) | fpt_stats sink (104 B) | ticket sink (8 B)
+constexpr size_t kNoAllocSlotsOff = kNoAllocHeader;
+constexpr size_t kNoAllocRingOff = kNoAllocSlotsOff + (size_t)kNoAllocMaxTraj * sizeof(ParkSlot);
+constexpr size_t kNoAllocRingEntries = (size_t)(kNoAllocMaxTraj + kNoAllocMaxGrid);      // grid x ceil(n / grid) <= n + grid - 1
+constexpr size_t kNoAllocBytes = kNoAllocRingOff + kNoAllocRingEntries * sizeof(unsigned long long);
+static_assert(sizeof(DevStats) <= 128 && sizeof(fpt_stats) <= 256 - 8, "header layout");
+static_assert(kNoAllocBytes < (6u << 20), "the scratch array is meant to stay modest");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocBytes];
+
+struct NoAllocCtx {           // per device: the array's DEVICE address (the name above is only a host-side handle) and the SM count
+  std::atomic<bool> ready{false};
+  unsigned char* base = nullptr;
+  int sm_count = 0;
+};
+NoAllocCtx g_noalloc[kMaxDevices];
+std::mutex g_noalloc_mu;
+
+int noalloc_ctx(NoAllocCtx** out) {
+  int dev = 0;
+  FPT_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return FPT_E_CUDA;
+  NoAllocCtx& c = g_noalloc[dev];
+  if (!c.ready.load(std::memory_order_acquire)) {
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!c.ready.load(std::memory_order_relaxed)) {
+      void* ptr = nullptr;                                          // with device `dev` current: this device's copy of the array
+      FPT_CUDA(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+      if (!ptr) return FPT_E_CUDA;
+      c.base = (unsigned char*)ptr;
+      FPT_CUDA(cudaDeviceGetAttribute(&c.sm_count, cudaDevAttrMultiProcessorCount, dev));
+      c.ready.store(true, std::memory_order_release);
+    }
+  }
+  *out = &c;
+  return FPT_OK;
+}
+
+}  // namespace
+
+extern "C" int fpt_simulate_noalloc(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt,
+                                    double* out_gamma, int32_t* out_status, fpt_stats* d_stats, void* cuda_stream) {
+  int rc = validate(p, n_traj, t_max);
+  if (rc != FPT_OK) return rc;
+  if (n_traj > 0 && (!out_fpt || !out_status)) return FPT_E_INVALID;
+  if ((unsigned long long)n_traj > kNoAllocMaxTraj) return FPT_E_TOO_LARGE;
+  if (n_traj == 0) return FPT_OK;
+  cudaStream_t stream = (cudaStream_t)cuda_stream;
+  NoAllocCtx* ctx = nullptr;
+  if ((rc = noalloc_ctx(&ctx)) != FPT_OK) return rc;
+  const int sms = ctx->sm_count;
+
+  KParams P;
+  derive(*p, t_max, seed, P);
+  P.n_traj = (unsigned long long)n_traj;
+  P.out_fpt = out_fpt;
+  P.out_gamma = out_gamma;
+  P.out_status = out_status;
+  DevStats* ws = (DevStats*)ctx->base;
+  fpt_stats* sink = (fpt_stats*)(ctx->base + 128);
+  unsigned long long* sink_ticket = (unsigned long long*)(ctx->base + 256 - 8);
+  FPT_CUDA(cudaMemsetAsync(ws, 0, 128, stream));                    // id counter and statistics start at zero
+  P.ws = ws;
+
+  int grid = 1, block = 128, kernel = FPT_KERNEL_FILL;
+  const bool fp32 = p->precision != FPT_PREC_FP64;
+  const bool strict = p->scheme == FPT_SCHEME_PAPER;
+  const bool at_once_escaped = fp32 ? (strict ? !((float)p->phi0 <= (float)p->threshold) : !((float)p->phi0 < (float)p->threshold))
+                                    : (strict ? !(p->phi0 <= p->threshold) : !(p->phi0 < p->threshold));
+  if (at_once_escaped || P.n_cap == 0) {
+    block = 256;
+    grid = (int)std::min<int64_t>((n_traj + block - 1) / block, (int64_t)sms * 8);
+    const double gam = std::fma(P.dgamma, at_once_escaped ? 0.0 : (double)P.n_cap, P.gamma0);
+    fpt_fill_kernel<<<grid, block, 0, stream>>>(P, at_once_escaped ? kStatusEscaped : kStatusCensored, at_once_escaped ? 0.0 : -1.0, gam);
+    FPT_CUDA(cudaGetLastError());
+  } else {
+    const bool amp = p->amp != 0.0, ramp = p->nu != 0.0;
+    const void* fn = p->precision == FPT_PREC_FP32_FAST ? persistent_kernel_f32_fast(p->model, ramp)
+                     : fp32                            ? persistent_kernel_f32(p->model, p->scheme, amp, ramp)
+                                                       : persistent_kernel_f64(p->model, p->scheme, amp, ramp);
+    int per_sm = 0;
+    FPT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, block, 0));
+    if (per_sm < 1) return FPT_E_CUDA;
+    // blocks of 128: all trajectories of a ramped job in flight if they fit, a fifth of a constant-bias job (as the
+    // allocating path, without its refinements), at least one block per SM, never more lanes than trajectories
+    const long long unit = 128LL * sms;
+    long long units = ramp ? (n_traj + unit - 1) / unit : n_traj / (5 * unit);
+    units = std::max<long long>(1, std::min<long long>(units, per_sm));
+    const long long blocks = std::min<long long>(units * sms, (n_traj + block - 1) / block);
+    grid = (int)blocks;
+    kernel = FPT_KERNEL_PERSISTENT;
+    // equal-length trajectories on fewer lanes: rotate them through the parking slots of the array (time slicing)
+    if (ramp && (long long)grid * block < n_traj && P.n_cap >= (1ull << 15)) {
+      unsigned long long q = 2048;
+      while (q < (unsigned long long)P.K || q * 2048ull < P.n_cap) q <<= 1;
+      if ((q % (unsigned long long)P.K) != 0ull) q *= (unsigned long long)P.K;
+      const unsigned long long cap = ((unsigned long long)n_traj + (unsigned long long)grid - 1ull) / (unsigned long long)grid;
+      if ((q & (q - 1ull)) == 0ull && (unsigned long long)grid * cap <= kNoAllocRingEntries) {
+        P.slice_cap = cap;
+        P.slice_slots = (ParkSlot*)(ctx->base + kNoAllocSlotsOff);
+        P.slice_ring = (unsigned long long*)(ctx->base + kNoAllocRingOff);
+        FPT_CUDA(cudaMemsetAsync(P.slice_ring, 0, (size_t)grid * (size_t)cap * sizeof(unsigned long long), stream));   // 0 = not published
+        P.slice_mask = q - 1ull;
+      }
+    }
+    P.schedule = FPT_SCHEDULE_DYNAMIC;
+    P.tail_helper = 1;
+    void* args[] = {(void*)&P};
+    FPT_CUDA(cudaLaunchKernel(fn, dim3(grid), dim3(block), args, 0, stream));
+  }
+  fpt_stats geo{};
+  geo.n_traj = (uint64_t)n_traj;
+  geo.n_cap = P.n_cap;
+  geo.grid = grid;
+  geo.block = block;
+  geo.check_every = P.K;
+  geo.kernel = kernel;
+  fpt_export_stats_kernel<<<1, 1, 0, stream>>>(ws, geo, d_stats, sink, sink_ticket, 0ull);
+  FPT_CUDA(cudaGetLastError());
+  return FPT_OK;
+}

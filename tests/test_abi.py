@@ -47,6 +47,7 @@ def test_strerror(lib):
     assert lib.fpt_strerror(0) == b"ok"
     assert lib.fpt_strerror(-1) == b"invalid argument"
     assert lib.fpt_strerror(-99) == b"unknown error code"
+    assert b"beyond the fixed maximum" in lib.fpt_strerror(-3)
 
 
 def _good():
@@ -111,6 +112,13 @@ def test_invalid_call_arguments(lib):
     assert ex(None, fpt.FptHist(0, 10, 0.0, 1.0, None)) == -1
     assert lib.fpt_simulate_ex(C.byref(p), 0, 1, 1.0, None, None, None, None, None, None, None) == 0
     assert lib.fpt_set_specialise(2, 0, 0) == -1 and lib.fpt_set_specialise(0, 0, 0) == 0
+    # fpt_simulate_noalloc: the fixed maximum and the argument checks come before any CUDA work
+    na = lambda n, f=C.c_void_p(8), st=C.c_void_p(8), pp=C.byref(p): lib.fpt_simulate_noalloc(pp, n, 1, 1.0, f, None, st, None, None)
+    assert na(binding.NOALLOC_MAX_TRAJ + 1) == -3 and na(1 << 40) == -3
+    assert na(-1) == -1 and na(10, None) == -1 and na(10, C.c_void_p(8), None) == -1 and na(10, pp=None) == -1
+    assert na(0, None, None) == 0
+    header = (ROOT / "include" / "fpt.h").read_text()
+    assert f"#define FPT_NOALLOC_MAX_TRAJ {binding.NOALLOC_MAX_TRAJ}\n" in header
     assert lib.fpt_dbg_set_slice_quantum(96) == -1 and lib.fpt_dbg_set_slice_quantum(64) == 0 and lib.fpt_dbg_set_slice_quantum(0) == 0
     assert lib.fpt_set_launch(48, 0, 0) == -1
     assert lib.fpt_set_launch(512, 0, 0) == -1
@@ -139,3 +147,16 @@ def test_product_does_not_import_oracle():
             text = path.read_text()
             assert "import oracle" not in text and "from oracle" not in text, path
             assert "fpt_oracle" not in text, path
+
+
+def test_noalloc_entry_point_has_no_allocating_call_and_takes_its_scratch_address_from_the_symbol():
+    """fpt_simulate_noalloc and its set-up (the last section of fpt_api.cu): no cudaMalloc / cudaFree / pool call, no use of
+    device_ctx() (whose first call per device allocates), the scratch is one static __device__ __align__(256) array, and host
+    code reaches it through cudaGetSymbolAddress only."""
+    src = (ROOT / "paper_1802_05065_b200" / "csrc" / "fpt_api.cu").read_text()
+    sec = src[src.index("// fpt_simulate_noalloc (fpt.h)"):]
+    code = re.sub(r"//[^\n]*", "", re.sub(r"/\*.*?\*/", "", sec, flags=re.S))
+    for banned in ("cudaMalloc", "cudaFree", "cudaMemPool", "device_ctx(", "WsGuard", "cudaHostAlloc", "cudaStreamCreate", "cudaEventCreate"):
+        assert banned not in code, banned
+    assert re.search(r"static __device__ __align__\(256\) unsigned char g_noalloc_scratch\[kNoAllocBytes\];", code)
+    assert code.count("g_noalloc_scratch") == 2 and "cudaGetSymbolAddress(&ptr, g_noalloc_scratch)" in code

@@ -130,14 +130,15 @@ typedef struct fpt_launch_opts {
                              the dynamic schedule; otherwise the persistent kernel runs.                                  */
   int32_t consumers;      /* specialised kernel: consumer warps per block, 1..4 (0 = default)                           */
   int32_t producers;      /* specialised kernel: producer warps per consumer, 1..3 (0 = default)                        */
-  int32_t time_slice;     /* persistent kernel, dynamic schedule, more trajectories than resident lanes: 0 = automatic (ramped
-                             jobs, whose trajectories are equally long, of one to three ragged "waves", and ramped fp32 jobs
-                             of 3 to 3.8 blocks of 128 per SM, which then run 3 blocks per SM), 1 = always, -1 = never.  Block b
-                             then owns the trajectories b, b + grid, ...; a lane sets its trajectory aside in device memory
-                             (32 B per trajectory + 8 B per ring entry, from the call's stream-ordered pool) after a quantum
-                             of >= 2048 steps while others of its block's are waiting and takes the one that has waited
-                             longest (round robin), so that all trajectories advance at the same rate and no ragged last
-                             wave idles the GPU.  Results are the same bits either way.                                  */
+  int32_t time_slice;     /* persistent kernel, dynamic schedule, RAMPED bias (nu != 0: trajectories about equally long), more
+                             trajectories than resident lanes: 0 = automatic (jobs of one to three ragged "waves", and fp32
+                             jobs of 3 to 3.8 blocks of 128 per SM, which then run 3 blocks per SM), 1 = always, -1 = never.
+                             Block b then owns the trajectories b, b + grid, ...; a lane sets its trajectory aside in device
+                             memory (32 B per trajectory + 8 B per ring entry, from the call's stream-ordered pool) after a
+                             quantum of >= 2048 steps while others of its block's are waiting and takes the one that has
+                             waited longest (round robin), so that all trajectories advance at the same rate and no ragged
+                             last wave idles the GPU.  Results are the same bits either way.  Ignored for a constant bias
+                             (exponentially distributed lengths: the refill balances those).                          */
   int32_t reserved;       /* must be 0 */
 } fpt_launch_opts;
 

@@ -320,7 +320,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     const void* fn = nullptr;
     size_t smem = hist_bytes;
     long long blocks = 0;
-    bool want_slice = cfg.time_slice == 1;
+    bool want_slice = cfg.time_slice == 1 && ramp;     // the slicing code exists in the ramped-bias kernels only (State::kSlicing)
     if (spec) {
       size_t fixed = 0, chan = 0;
       fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &fixed, &chan)

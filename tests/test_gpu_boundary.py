@@ -81,13 +81,15 @@ def test_specialised_kernel_every_layout_matches_the_oracle(name, w, n):
 def test_time_slicing_rotates_trajectories_without_changing_results():
     """fpt_launch_opts.time_slice: with fewer lanes than trajectories, a lane sets its trajectory aside in device memory every
     quantum (2048 steps or more) while others of its block's wait and takes the one that has waited longest.  A set-aside trajectory resumes from (phi, v[, t, c],
-    k) with its Philox position, ramp registers and Kahan pair rebuilt: results stay the oracle's bit for bit -- ramped and
-    constant bias, fp64 and fp32, with the fused histogram -- and the rotation really happens."""
+    k) with its Philox position, ramp registers and Kahan pair rebuilt: results stay the oracle's bit for bit -- narrow and wide
+    spreads of the trajectory lengths, Heun and Euler, fp64 and fp32, with the fused histogram -- and the rotation really happens.
+    The code is compiled into the ramped-bias kernels only: for a constant bias the option is ignored."""
     cases = [
         (fpt.workload("c3", nu=2e-4, t_max=1.05 / 2e-4), 700, True),                         # fp64 ramp, ~2.4e5 steps each
         (fpt.workload("c4", nu=2e-5, t_max=0.55 / 2e-5), 900, True),                         # fp32 + Kahan time, ~3.6e5 steps
-        (fpt.workload("c2", t_max=400.0), 3000, False),                                      # constant bias: finishes and preemptions mix
-        (fpt.workload("c5", temperature=0.1, t_max=1500.0), 2500, False),                    # EM overdamped, some censored
+        (fpt.workload("c2", nu=1e-4, t_max=120.0), 3000, False),                             # hot, slow ramp: widely spread lengths, so finishes,
+                                                                                             # refills and preemptions mix; some censored
+        (fpt.workload("c5", temperature=0.1, nu=2e-5, t_max=1000.0), 2500, False),           # EM overdamped, ramped, some censored
     ]
     for w, n, hist in cases:
         ora = _oracle(w, n)
@@ -110,6 +112,11 @@ def test_time_slicing_rotates_trajectories_without_changing_results():
         fpt.dbg_set_slice_quantum(0)
     _assert_oracle(out, ora, w)
     assert st["time_slices"] > 20 * n, st
+    # constant bias: ignored (State::kSlicing), same results
+    wc = fpt.workload("c2", t_max=60.0)
+    out, st = _ex(wc, 2000, fpt.launch_opts(specialise=False, time_slice=True, block=64, blocks_per_sm=1, max_blocks=5))
+    _assert_oracle(out, _oracle(wc, 2000), None)
+    assert st["time_slices"] == 0
     # all trajectories resident: nothing ever waits, nothing is set aside
     w = fpt.workload("c3", nu=2e-3, t_max=1.05 / 2e-3)
     out, st = _ex(w, 256, fpt.launch_opts(specialise=False, time_slice=True, block=128, blocks_per_sm=1))

@@ -425,7 +425,7 @@ def test_random_geometries_poll_intervals_and_helper_settings_agree():
     the first run, bit for bit -- the outputs are a function of (params, seed, id) only."""
     rng = np.random.default_rng(99)
     for w, n in [(fpt.workload("c2", t_max=90.0), 5000), (fpt.workload("c5", temperature=0.12, t_max=250.0), 4000),
-                 (fpt.workload("c4", nu=2e-4, t_max=2220.0), 3000)]:
+                 (fpt.workload("c4", nu=2e-4, t_max=2220.0), 3000), (fpt.workload("c3", nu=1.5e-3, t_max=665.0), 2500)]:
         ref = run_gpu(w, n)
         assert 0 < np.sum(ref[2] == 1) < n and np.sum(ref[2] == 0) > 0
         for trial in range(int(os.environ.get("FPT_STRESS_TRIALS", "40"))):

@@ -243,6 +243,13 @@ int ensure_dynamic_smem(const void* fn, size_t dyn_bytes, int dev) {
   return FPT_OK;
 }
 
+// the persistent kernel with the time-slicing code (ramped-bias states only)
+const void* sliced_kernel(const fpt_params* p, bool amp) {
+  if (p->precision == FPT_PREC_FP32_FAST) return persistent_sliced_kernel_f32_fast(p->model);
+  return p->precision != FPT_PREC_FP64 ? persistent_sliced_kernel_f32(p->model, p->scheme, amp)
+                                       : persistent_sliced_kernel_f64(p->model, p->scheme, amp);
+}
+
 int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_max, double* out_fpt, double* out_gamma,
                   int32_t* out_status, const fpt_hist* hist, const fpt_launch_opts* opts_in, fpt_stats* d_stats,
                   void* cuda_stream) {
@@ -320,7 +327,7 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
     const void* fn = nullptr;
     size_t smem = hist_bytes;
     long long blocks = 0;
-    bool want_slice = cfg.time_slice == 1 && ramp;     // the slicing code exists in the ramped-bias kernels only (State::kSlicing)
+    bool want_slice = cfg.time_slice == 1 && ramp;     // the slicing kernels exist for the ramped-bias states only
     if (spec) {
       size_t fixed = 0, chan = 0;
       fn = fp32 ? specialised_kernel_f32(p->model, p->scheme, ramp, &fixed, &chan)
@@ -420,6 +427,13 @@ int simulate_impl(const fpt_params* p, int64_t n_traj, uint64_t seed, double t_m
       }
       if ((q % (unsigned long long)P.K) != 0ull) q *= (unsigned long long)P.K;       // K not a power of two: any multiple will do
       if ((q & (q - 1ull)) == 0ull) {
+        fn = sliced_kernel(p, amp);                                 // the variant of the kernel that holds the slicing code
+        rc = ensure_dynamic_smem(fn, smem, dev);
+        if (rc != FPT_OK) return rc;
+        int per_sm_s = 0;
+        FPT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_s, fn, block, smem));
+        if (per_sm_s < 1) return FPT_E_CUDA;
+        if ((long long)per_sm_s * sms < (long long)grid) grid = per_sm_s * sms;       // all blocks resident (slicing balances any grid)
         P.slice_cap = ((unsigned long long)n_traj + (unsigned long long)grid - 1ull) / (unsigned long long)grid;
         const size_t slot_bytes = (size_t)n_traj * sizeof(ParkSlot);
         const size_t ring_bytes = (size_t)grid * (size_t)P.slice_cap * sizeof(unsigned long long);
@@ -1066,7 +1080,11 @@ extern "C" int fpt_simulate_noalloc(const fpt_params* p, int64_t n_traj, uint64_
       while (q < (unsigned long long)P.K || q * 2048ull < P.n_cap) q <<= 1;
       if ((q % (unsigned long long)P.K) != 0ull) q *= (unsigned long long)P.K;
       const unsigned long long cap = ((unsigned long long)n_traj + (unsigned long long)grid - 1ull) / (unsigned long long)grid;
-      if ((q & (q - 1ull)) == 0ull && (unsigned long long)grid * cap <= kNoAllocRingEntries) {
+      const void* fn_s = sliced_kernel(p, amp);
+      int per_sm_s = 0;
+      FPT_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_s, fn_s, block, 0));
+      if ((q & (q - 1ull)) == 0ull && (unsigned long long)grid * cap <= kNoAllocRingEntries && (long long)per_sm_s * sms >= (long long)grid) {
+        fn = fn_s;
         P.slice_cap = cap;
         P.slice_slots = (ParkSlot*)(ctx->base + kNoAllocSlotsOff);
         P.slice_ring = (unsigned long long*)(ctx->base + kNoAllocRingOff);

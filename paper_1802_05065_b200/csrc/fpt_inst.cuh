@@ -10,6 +10,10 @@ namespace fpt {
 // persistent integrator for (model, scheme, amp != 0, nu != 0)
 const void* persistent_kernel_f64(int model, int scheme, bool amp, bool ramp);
 const void* persistent_kernel_f32(int model, int scheme, bool amp, bool ramp);
+// the same with the time-slicing code (ramped bias only: nu != 0)
+const void* persistent_sliced_kernel_f64(int model, int scheme, bool amp);
+const void* persistent_sliced_kernel_f32(int model, int scheme, bool amp);
+const void* persistent_sliced_kernel_f32_fast(int model);
 // warp-specialised integrator (drifts with a sine only: amp != 0); dynamic shared memory = *fixed_bytes + consumers x
 // *channel_bytes (+ the histogram bins)
 const void* specialised_kernel_f64(int model, int scheme, bool ramp, size_t* fixed_bytes, size_t* channel_bytes);

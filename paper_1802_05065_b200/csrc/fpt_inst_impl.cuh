@@ -11,6 +11,8 @@ template <template <int, int, bool, bool> class St>
 struct Inst {
   template <int M, int S, bool A, bool R>
   static const void* pk() { return (const void*)&fpt_persistent_kernel<St<M, S, A, R>>; }
+  template <int M, int S, bool A>
+  static const void* pks() { return (const void*)&fpt_persistent_kernel<St<M, S, A, true>, true>; }      // with time slicing: ramped only
   template <int M, int S, bool A, bool R>
   static const void* tk() { return (const void*)&fpt_trace_kernel<St<M, S, A, R>>; }
   template <int M, int S, bool R>
@@ -34,6 +36,13 @@ struct Inst {
     if (model == 0) return scheme == 0 ? pick_p<0, 0>(a, r) : scheme == 1 ? pick_p<0, 1>(a, r) : pick_p<0, 2>(a, r);
     return scheme == 0 ? pick_p<1, 0>(a, r) : scheme == 1 ? pick_p<1, 1>(a, r) : pick_p<1, 2>(a, r);
   }
+  template <int M, int S>
+  static const void* pick_ps(bool a) { return a ? pks<M, S, true>() : pks<M, S, false>(); }
+  static const void* persistent_sliced(int model, int scheme, bool a) {
+    if (model == 0) return scheme == 0 ? pick_ps<0, 0>(a) : scheme == 1 ? pick_ps<0, 1>(a) : pick_ps<0, 2>(a);
+    return scheme == 0 ? pick_ps<1, 0>(a) : scheme == 1 ? pick_ps<1, 1>(a) : pick_ps<1, 2>(a);
+  }
+  static const void* persistent_sliced_paper(int model) { return model == 0 ? pks<0, 2, true>() : pks<1, 2, true>(); }
   static const void* trace(int model, int scheme, bool a, bool r) {
     if (model == 0) return scheme == 0 ? pick_t<0, 0>(a, r) : scheme == 1 ? pick_t<0, 1>(a, r) : pick_t<0, 2>(a, r);
     return scheme == 0 ? pick_t<1, 0>(a, r) : scheme == 1 ? pick_t<1, 1>(a, r) : pick_t<1, 2>(a, r);

@@ -110,16 +110,16 @@ def count() -> dict:
     table = {}
     for mangled, instrs in funcs.items():
         name = names[mangled]
-        m = re.search(r"fpt_(persistent|specialised)_kernel<fpt::State(64|32)(?:X)?<(\d), ?(\d), ?(true|false), ?(true|false)(?:, ?(true|false))?>", name)
+        m = re.search(r"fpt_(persistent|specialised)_kernel<fpt::State(64|32)(?:X)?<(\d), ?(\d), ?(true|false), ?(true|false)(?:, ?(true|false))? ?>(, ?true)?", name)
         if not m:
             continue
-        kind, prec, model, scheme, amp, ramp, fast = m.groups()
+        kind, prec, model, scheme, amp, ramp, fast, sliced = m.groups()
         fp32 = prec == "32"
         macro = 4 if fp32 else 2
         loops = [(s, e, _classify(instrs[s:e + 1])) for (s, e) in _loops(instrs)]
         loops = [l for l in loops if l[2]["fp64"] + l[2]["fp32"] >= 8]
         loops.sort(key=lambda l: -(l[2]["fp64"] + l[2]["fp32"]))
-        key = f"{kind}_f{prec}_{'ud' if model == '1' else 'od'}_{('em', 'heun', 'paper')[int(scheme)]}_{'sin' if amp == 'true' else 'nosin'}_{'ramp' if ramp == 'true' else 'const'}" + ("_hwsin" if fast == "true" else "")
+        key = f"{kind}_f{prec}_{'ud' if model == '1' else 'od'}_{('em', 'heun', 'paper')[int(scheme)]}_{'sin' if amp == 'true' else 'nosin'}_{'ramp' if ramp == 'true' else 'const'}" + ("_hwsin" if fast == "true" else "") + ("_sliced" if sliced else "")
         entry = {"kernel": name.split("(")[0]}
 
         def per_step(c, steps):

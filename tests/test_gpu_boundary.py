@@ -83,7 +83,7 @@ def test_time_slicing_rotates_trajectories_without_changing_results():
     quantum (2048 steps or more) while others of its block's wait and takes the one that has waited longest.  A set-aside trajectory resumes from (phi, v[, t, c],
     k) with its Philox position, ramp registers and Kahan pair rebuilt: results stay the oracle's bit for bit -- narrow and wide
     spreads of the trajectory lengths, Heun and Euler, fp64 and fp32, with the fused histogram -- and the rotation really happens.
-    The code is compiled into the ramped-bias kernels only: for a constant bias the option is ignored."""
+    The slicing variant of the kernel exists for the ramped-bias states only: for a constant bias the option is ignored."""
     cases = [
         (fpt.workload("c3", nu=2e-4, t_max=1.05 / 2e-4), 700, True),                         # fp64 ramp, ~2.4e5 steps each
         (fpt.workload("c4", nu=2e-5, t_max=0.55 / 2e-5), 900, True),                         # fp32 + Kahan time, ~3.6e5 steps
@@ -112,7 +112,7 @@ def test_time_slicing_rotates_trajectories_without_changing_results():
         fpt.dbg_set_slice_quantum(0)
     _assert_oracle(out, ora, w)
     assert st["time_slices"] > 20 * n, st
-    # constant bias: ignored (State::kSlicing), same results
+    # constant bias: ignored (no slicing variant of those kernels), same results
     wc = fpt.workload("c2", t_max=60.0)
     out, st = _ex(wc, 2000, fpt.launch_opts(specialise=False, time_slice=True, block=64, blocks_per_sm=1, max_blocks=5))
     _assert_oracle(out, _oracle(wc, 2000), None)

@@ -73,7 +73,7 @@ typedef struct fpt_params {
                             2 FPT_PREC_FP32_FAST */
   int32_t  check_every;  /* K >= 1: poll/refill interval in steps.  NEVER changes results (the crossing test is per step,
                             PAPER.md:190).  Rounded up to a multiple of the steps per Philox block (2 fp64, 4 fp32).
-                            0 = library default. */
+                            0 = library default (64; 128 for long caps; 512 for ramped trajectories of 2^22 steps or more). */
   double   alpha;        /* damping (paper beta); ignored for model 0 */
   double   temperature;  /* T (paper theta; D = beta*theta).  model 0: the diffusion constant */
   double   amp;          /* amplitude of sin phi; 0 => drifted Brownian motion with mu = gamma0 */

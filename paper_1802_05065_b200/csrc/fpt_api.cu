@@ -39,6 +39,12 @@ constexpr int kMaxDevices = 64;
 // fp32 64, and 128 from caps of 2^16 steps (config 4 twin: +3.8 % over 32; 256 is no better)
 constexpr int kDefaultK = 64, kDefaultKLong = 128;
 constexpr unsigned long long kLongCap64 = 1ull << 21, kLongCap32 = 1ull << 16;
+// ramped bias: a trajectory switches before the tilt reaches the critical one, after about (amp - gamma0) / (nu dt) steps,
+// so its length is known in advance to within the switching width.  From 2^22 steps a poll every 512 costs a finished lane
+// 256 idle steps in millions and saves three quarters of the polls (measured on B200 against 128: config 4's geometry
+// +1.2 % issued-lane throughput, config 3 as stated +0.2 %; 2048: +0.5 % on config 3, no better in fp32)
+constexpr int kDefaultKRampLong = 512;
+constexpr double kRampLongSteps = 4194304.0;
 // specialised kernel (fpt_specialised.cuh): hand-over chunk = its poll interval; limits of fpt_launch_opts
 constexpr int kSpecChunk64 = 64, kSpecChunk32 = 32;
 constexpr int kSpecMaxConsumersHost = 4, kSpecMaxProducersHost = 3;
@@ -170,6 +176,9 @@ void derive(const fpt_params& p, double t_max, uint64_t seed, KParams& P) {
   const int macro = p.precision != FPT_PREC_FP64 ? 4 : 2;
   const unsigned long long long_cap = p.precision != FPT_PREC_FP64 ? kLongCap32 : kLongCap64;
   int K = p.check_every > 0 ? p.check_every : (P.n_cap >= long_cap ? kDefaultKLong : kDefaultK);
+  if (p.check_every <= 0 && p.nu > 0.0 && p.amp > p.gamma0 &&
+      std::fmin((double)P.n_cap, (p.amp - p.gamma0) / (p.nu * p.dt)) >= kRampLongSteps)
+    K = kDefaultKRampLong;
   K = ((K + macro - 1) / macro) * macro;
   P.K = K;
   P.hist_of = -1;

@@ -150,6 +150,27 @@ def test_time_slicing_is_the_default_where_equal_length_trajectories_leave_a_rag
     assert st["time_slices"] == 0
 
 
+def test_default_poll_interval_follows_what_the_host_knows_about_the_trajectory_length():
+    """check_every = 0: 64; 128 from long caps (2^21 steps fp64, 2^16 fp32); 512 when the bias is ramped and the ramp reaches
+    the critical tilt (or the cap) only after 2^22 steps or more -- the length of a ramped trajectory is known in advance.
+    Never changes results."""
+    persistent = fpt.launch_opts(specialise=False)
+    w = fpt.workload("c3", t_max=4.3e6 * 0.02)                         # config 3's own ramp (nu = 1e-6), cut at 4.3e6 steps: all censored
+    out, st = _ex(w, 32, persistent)
+    assert st["check_every"] == 512 and st["n_censored"] == 32, st
+    _assert_oracle(out, _oracle(w, 32), None)
+    out128, st128 = _ex(w, 32, persistent, check_every=128)
+    assert st128["check_every"] == 128 and all(np.array_equal(a, b) for a, b in zip(out, out128))
+    _, st = _ex(fpt.workload("c3", nu=1e-3, t_max=1050.0), 64, persistent)                  # 5e4 steps to the critical tilt
+    assert st["check_every"] == 64
+    _, st = _ex(fpt.workload("c3", nu=1e-5, t_max=50.0), 64, persistent)                    # long ramp, short cap
+    assert st["check_every"] == 64
+    _, st = _ex(fpt.workload("c2", t_max=5.0), 64, persistent)                              # constant bias, cap 500 steps
+    assert st["check_every"] == 64
+    _, st = _ex(fpt.workload("c4", nu=1e-4, t_max=5500.0), 64, persistent)                  # fp32, cap 1.1e5 steps
+    assert st["check_every"] == 128
+
+
 def test_specialised_kernel_is_the_default_for_small_jobs_only():
     w = fpt.workload("c2", t_max=60.0)
     out, st = _ex(w, 4000)
